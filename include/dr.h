@@ -1,0 +1,130 @@
+/*
+ * dr.h -- C ABI of libdr: pseudo-transient (PT) solver for quasi-static linear elasticity on a 3-D voxel
+ * image and the six-load-case driver that returns the effective 6x6 stiffness tensor (arXiv 2410.20441).
+ *
+ * Citations: P:NNN = PAPER.md line NNN of the paper text; "Reading Rn" = DESIGN.md section 3.
+ *
+ * Problem (sec. 2): div sigma = 0, sigma = C(x):eps(u) on a cuboid of nx*ny*nz cubic voxels of
+ * size h with bulk modulus K and shear modulus G per voxel; apply a uniform strain through displacement
+ * ("velocity", physical step Delta t = 1) boundary conditions (sec. 3.4, App. A);
+ * <sigma> = C* <eps> (Eq. 7-9) gives one column of C* per load case.
+ * Method (sec. 3.1): accelerated pseudo-transient iteration, Eq. 10-21, on a staggered grid
+ * (sec. 3.3): normal stresses and moduli at cell centres, velocities on faces, shear stresses on edges.
+ *
+ * Conventions
+ *  - All arrays are fp64, x fastest: index = i + nx*(j + ny*k) for the nx*ny*nz cell fields.
+ *  - Voigt order xx,yy,zz,yz,xz,xy ("C55 (xz)" P:365); engineering shear strain gamma = 2 eps.
+ *  - Load cases 0..5 apply the displacement gradient D with one non-zero entry eps0:
+ *      0: Dxx  1: Dyy  2: Dzz  (normal compression tests, App. A.1)
+ *      3: u_y = eps0 z   4: u_x = eps0 z   5: u_x = eps0 y   (simple shear tests, App. A.2)
+ *  - Units of C* are the units of K and G.
+ *  - The library allocates NO device memory: the caller passes one workspace of dr_workspace_bytes() bytes
+ *    (e.g. a torch tensor) that is borrowed until dr_destroy.  K and G are borrowed during dr_create only.
+ *  - Every launch goes to the cuda_stream given at dr_create (a cudaStream_t cast to void*, NULL = default
+ *    stream).  Calls that return host values synchronise that stream.
+ *  - Errors are return codes, never exceptions or aborts.  dr_last_error() gives a message for the last
+ *    non-OK status of that handle.  DR_MAXITER is a soft status: fields, averages and the C column are
+ *    valid and stored.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns DR_ERR_CUDA.
+ */
+#ifndef DR_H
+#define DR_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dr_handle dr_handle;            /* opaque, owned by the library */
+
+typedef enum {
+    DR_OK = 0,
+    DR_ERR_ARG = 1,         /* invalid argument (sizes, h<=0, eps0==0, tol<=0, negative/NaN moduli, ...)   */
+    DR_ERR_WORKSPACE = 2,   /* workspace NULL, misaligned (needs 256 B) or smaller than dr_workspace_bytes */
+    DR_ERR_CUDA = 3,        /* a CUDA runtime call failed (message in dr_last_error)                      */
+    DR_ERR_DIVERGED = 4,    /* residual became NaN/Inf                                                     */
+    DR_ERR_STATE = 5,       /* call order (e.g. dr_effective_C before six columns exist)                   */
+    DR_MAXITER = 6          /* soft: maxiter reached before res <= tol                                     */
+} dr_status;
+
+/* dr_set_param ids.  Defaults in brackets. */
+typedef enum {
+    DR_CFL = 0,        /* C~ of Eq. 14 P:98 [0.55]; the 3-D stability limit is 1/sqrt(3) (Reading R10)        */
+    DR_ST_FACTOR = 1,  /* St = 2 pi sqrt(3) * factor, Eq. 16, 21 P:107-130 [1.0]                               */
+    DR_NCHECK = 2,     /* residual is evaluated every ncheck iterations [50]                                  */
+    DR_GAVG = 3,       /* shear modulus on edges: 0 harmonic mean of the 4 cells [default], 1 arithmetic (R4) */
+    DR_VOID_REL = 4,   /* r>0: cells with K+4G/3 <= r*max(K+4G/3) become exact void K=G=0 [0 = off] (R9)      */
+    DR_BC_MODE = 5,    /* 0 paper's mixed BCs [default]; 1 full kinematic uniform BC on all faces (R5)        */
+    DR_KERNEL = 6      /* 0 fused z-march kernel [default]; 1 split stress/velocity kernels (baseline)        */
+} dr_param;
+
+/* Bytes of device workspace dr_create needs for an nx*ny*nz grid (0 if the sizes are invalid). */
+size_t dr_workspace_bytes(int nx, int ny, int nz);
+
+/* Create a solver.  nx,ny,nz >= 2; h > 0.
+ * K, G: DEVICE pointers, nx*ny*nz doubles each, x fastest, >= 0 and finite (K = G = 0 is void, G = 0 with K > 0
+ * is a fluid; both allowed).  They are read (copied into the workspace with a replicate halo) and not kept.
+ * workspace: DEVICE pointer, 256-byte aligned, workspace_bytes >= dr_workspace_bytes(nx,ny,nz), borrowed until
+ * dr_destroy; its previous content is overwritten.  cuda_stream: cudaStream_t or NULL.
+ * Sets up the constants of Eq. 14-21.  On error *out = NULL. */
+dr_status dr_create(int nx, int ny, int nz, double h,
+                    const double* K, const double* G,
+                    void* workspace, size_t workspace_bytes,
+                    void* cuda_stream, dr_handle** out);
+
+/* Set a parameter (before dr_solve / dr_step). */
+dr_status dr_set_param(dr_handle* h, int id, double value);
+
+/* One load case: initial fields and boundary values (App. A), then PT iterations (Eq. 11-13) until the
+ * residual max-norm  res = max_nodes |div sigma| h / (H_node |eps0|)  <= tol, tested every ncheck iterations
+ * ("once the dynamic fields attenuate to a certain precision"), at most maxiter iterations; then the
+ * volume averages (Eq. 7) and column load_case of C* (Eq. 9, 22).  eps0 != 0, tol > 0, maxiter >= 1. */
+dr_status dr_solve(dr_handle* h, int load_case, double eps0, double tol, int maxiter);
+
+/* Same with a fixed iteration count and no convergence test (parity tests): initial fields, niter >= 0
+ * iterations, the residual of the last iteration, the volume averages and the (unconverged) column. */
+dr_status dr_step(dr_handle* h, int load_case, double eps0, int niter);
+
+/* Continue niter PT iterations from the current fields without residual or averages (throughput timing).
+ * Needs a previous dr_step/dr_solve with the same load case and eps0.  Does not synchronise the stream. */
+dr_status dr_iterate(dr_handle* h, int load_case, double eps0, int niter);
+
+/* Effective stiffness, HOST pointer, row-major out[6*m + n] = C*_mn (Voigt).  DR_ERR_STATE until all six
+ * load cases have been solved.  Not symmetrised. */
+dr_status dr_effective_C(dr_handle* h, double out[36]);
+
+/* Volume-averaged stresses of the last solve/step, HOST pointer, Voigt order (Eq. 7). */
+dr_status dr_avg_stress(dr_handle* h, double out[6]);
+
+/* Iterations done, last residual, and milliseconds (CUDA events on the stream, whole call) of the last
+ * dr_solve/dr_step.  Any pointer may be NULL. */
+dr_status dr_info(dr_handle* h, int* iters, double* residual, double* ms);
+
+/* Copy one field to a dense DEVICE array of its logical shape (x fastest, no pitch):
+ * field 0 vx (nx+1,ny,nz)   1 vy (nx,ny+1,nz)   2 vz (nx,ny,nz+1)   3 sxx  4 syy  5 szz (nx,ny,nz)
+ *       6 tyz (nx,ny+1,nz+1)   7 txz (nx+1,ny,nz+1)   8 txy (nx+1,ny+1,nz);   sigma_aa = -p + tau_aa (Eq. 10).
+ * n must equal the number of elements of that shape. */
+dr_status dr_get_field(dr_handle* h, int field, double* dst_device, size_t n);
+
+/* Whole 6x6 tensor from HOST arrays through the public API with host<->device copies inside: allocates
+ * nothing on the device itself -- K_host/G_host (nx*ny*nz doubles, pinned or pageable) are staged through
+ * stage_device (DEVICE, >= 2*nx*ny*nz doubles, caller-owned), then dr_create + 6 x dr_solve + dr_effective_C
+ * run in `workspace`.  C_out: HOST, 36 doubles.  iters_out: HOST, 6 ints or NULL.  Returns the worst status. */
+dr_status dr_solve_image_host(int nx, int ny, int nz, double h,
+                              const double* K_host, const double* G_host,
+                              double* stage_device, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                              double eps0, double tol, int maxiter, int ncheck,
+                              double C_out[36], int iters_out[6]);
+
+/* Number of kernel launches this handle has issued so far (for bench.py's gpu_launches). */
+long long dr_launch_count(dr_handle* h);
+
+const char* dr_last_error(dr_handle* h);
+
+void dr_destroy(dr_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DR_H */

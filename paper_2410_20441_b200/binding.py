@@ -1,0 +1,193 @@
+"""Thin Python binding of libdr (include/dr.h): argument marshalling only.
+
+PyTorch supplies device memory (workspace, K/G, exported fields) and the CUDA stream; every step of the
+path runs in the library's kernels.  There is no fallback: if libdr.so cannot be loaded or no CUDA device
+is present, construction raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdr.so")
+
+OK, ERR_ARG, ERR_WORKSPACE, ERR_CUDA, ERR_DIVERGED, ERR_STATE, MAXITER = range(7)
+CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL = range(7)
+PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL)
+FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
+EXPORTS = ("dr_workspace_bytes", "dr_create", "dr_set_param", "dr_solve", "dr_step", "dr_iterate",
+           "dr_effective_C", "dr_avg_stress", "dr_info", "dr_get_field", "dr_solve_image_host",
+           "dr_launch_count", "dr_last_error", "dr_destroy")
+
+_lib = None
+
+
+def lib():
+    """Load libdr.so (built in-tree by paper_2410_20441_b200.build).  Fails loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("libdr.so is not built: run `python -m paper_2410_20441_b200.build` "
+                               "(needs nvcc; there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        dp, vp = C.POINTER(C.c_double), C.c_void_p
+        L.dr_workspace_bytes.argtypes = [C.c_int] * 3
+        L.dr_workspace_bytes.restype = C.c_size_t
+        L.dr_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, vp, vp, vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.dr_set_param.argtypes = [vp, C.c_int, C.c_double]
+        L.dr_solve.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int]
+        L.dr_step.argtypes = [vp, C.c_int, C.c_double, C.c_int]
+        L.dr_iterate.argtypes = [vp, C.c_int, C.c_double, C.c_int]
+        L.dr_effective_C.argtypes = [vp, dp]
+        L.dr_avg_stress.argtypes = [vp, dp]
+        L.dr_info.argtypes = [vp, C.POINTER(C.c_int), dp, dp]
+        L.dr_get_field.argtypes = [vp, C.c_int, vp, C.c_size_t]
+        L.dr_solve_image_host.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, vp, vp, vp, vp, C.c_size_t, vp,
+                                          C.c_double, C.c_double, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
+        L.dr_launch_count.argtypes = [vp]
+        L.dr_launch_count.restype = C.c_longlong
+        L.dr_last_error.argtypes = [vp]
+        L.dr_last_error.restype = C.c_char_p
+        L.dr_destroy.argtypes = [vp]
+        L.dr_destroy.restype = None
+        _lib = L
+    return _lib
+
+
+class DrError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("libdr status %d: %s" % (status, msg))
+        self.status = status
+
+
+def workspace_bytes(nx, ny, nz):
+    return lib().dr_workspace_bytes(nx, ny, nz)
+
+
+def field_shape(nx, ny, nz, f):
+    return {0: (nz, ny, nx + 1), 1: (nz, ny + 1, nx), 2: (nz + 1, ny, nx),
+            3: (nz, ny, nx), 4: (nz, ny, nx), 5: (nz, ny, nx),
+            6: (nz + 1, ny + 1, nx), 7: (nz + 1, ny, nx + 1), 8: (nz, ny + 1, nx + 1)}[f]
+
+
+class Solver:
+    """dr_create .. dr_destroy.  K, G: torch.float64 CUDA tensors of shape (nz, ny, nx), x fastest."""
+
+    def __init__(self, K, G, h=1.0, stream=None, workspace=None, **params):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("libdr needs a CUDA device (there is no CPU fallback)")
+        if not (K.is_cuda and G.is_cuda and K.dtype == torch.float64 and G.dtype == torch.float64):
+            raise TypeError("K and G must be float64 CUDA tensors")
+        K = K.contiguous()
+        G = G.contiguous()
+        assert K.dim() == 3 and K.shape == G.shape
+        self.nz, self.ny, self.nx = (int(s) for s in K.shape)
+        self.device = K.device
+        self._torch = torch
+        need = workspace_bytes(self.nx, self.ny, self.nz)
+        if need == 0:
+            raise DrError(ERR_ARG, "invalid grid size")
+        if workspace is None:
+            workspace = torch.empty(need, dtype=torch.uint8, device=K.device)
+        self.workspace = workspace
+        self.stream = stream if stream is not None else torch.cuda.current_stream(K.device)
+        self._h = C.c_void_p()
+        with torch.cuda.device(K.device):
+            st = lib().dr_create(self.nx, self.ny, self.nz, float(h), K.data_ptr(), G.data_ptr(),
+                                 workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                 self.stream.cuda_stream, C.byref(self._h))
+        if st != OK:
+            raise DrError(st, "dr_create failed (status %d)" % st)
+        for k, v in params.items():
+            self.set_param(k, v)
+
+    def _check(self, st, soft=(OK,)):
+        if st not in soft:
+            raise DrError(st, lib().dr_last_error(self._h).decode())
+        return st
+
+    def set_param(self, name, value):
+        self._check(lib().dr_set_param(self._h, PARAM_IDS[name], float(value)))
+
+    def solve(self, lc, eps0=1e-4, tol=1e-8, maxiter=100000):
+        return self._check(lib().dr_solve(self._h, lc, eps0, tol, maxiter), soft=(OK, MAXITER))
+
+    def step(self, lc, eps0, niter):
+        return self._check(lib().dr_step(self._h, lc, eps0, niter))
+
+    def iterate(self, lc, eps0, niter):
+        return self._check(lib().dr_iterate(self._h, lc, eps0, niter))
+
+    def effective_C(self):
+        import numpy as np
+        out = np.zeros(36)
+        self._check(lib().dr_effective_C(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out.reshape(6, 6)
+
+    def avg_stress(self):
+        import numpy as np
+        out = np.zeros(6)
+        self._check(lib().dr_avg_stress(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def info(self):
+        it, r, ms = C.c_int(), C.c_double(), C.c_double()
+        lib().dr_info(self._h, C.byref(it), C.byref(r), C.byref(ms))
+        return it.value, r.value, ms.value
+
+    def get_field(self, f):
+        if isinstance(f, str):
+            f = FIELDS.index(f)
+        out = self._torch.empty(field_shape(self.nx, self.ny, self.nz, f), dtype=self._torch.float64, device=self.device)
+        self._check(lib().dr_get_field(self._h, f, out.data_ptr(), out.numel()))
+        return out
+
+    def launch_count(self):
+        return lib().dr_launch_count(self._h)
+
+    def solve_all(self, eps0=1e-4, tol=1e-8, maxiter=100000):
+        log = []
+        for lc in range(6):
+            st = self.solve(lc, eps0, tol, maxiter)
+            it, r, ms = self.info()
+            log.append((st, it, r, ms))
+        return self.effective_C(), log
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h:
+            lib().dr_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def solve_image_host(K_host, G_host, h=1.0, eps0=1e-4, tol=1e-8, maxiter=100000, ncheck=0,
+                     stage=None, workspace=None, device="cuda:0"):
+    """End-to-end call with HOST arrays (numpy or CPU torch tensors, (nz,ny,nx) float64): host->device copies,
+    six solves and the 6x6 result read back, all inside dr_solve_image_host.  Returns (C, iters, status)."""
+    import numpy as np
+    import torch
+    Kt = torch.as_tensor(K_host)
+    Gt = torch.as_tensor(G_host)
+    assert Kt.dtype == torch.float64 and Kt.is_contiguous() and Gt.is_contiguous() and not Kt.is_cuda
+    nz, ny, nx = (int(s) for s in Kt.shape)
+    N = nx * ny * nz
+    if stage is None:
+        stage = torch.empty(2 * N, dtype=torch.float64, device=device)
+    if workspace is None:
+        workspace = torch.empty(workspace_bytes(nx, ny, nz), dtype=torch.uint8, device=device)
+    Cout = np.zeros(36)
+    iters = (C.c_int * 6)()
+    with torch.cuda.device(stage.device):
+        st = lib().dr_solve_image_host(nx, ny, nz, float(h), Kt.data_ptr(), Gt.data_ptr(), stage.data_ptr(),
+                                       workspace.data_ptr(), workspace.numel(), torch.cuda.current_stream().cuda_stream,
+                                       eps0, tol, maxiter, ncheck, Cout.ctypes.data_as(C.POINTER(C.c_double)), iters)
+    if st not in (OK, MAXITER):
+        raise DrError(st, "dr_solve_image_host failed")
+    return Cout.reshape(6, 6), list(iters), st

@@ -1,0 +1,442 @@
+// dr_api.cu -- host side of libdr: the C ABI of include/dr.h (handle, workspace carving, PT constants of
+// Eq. 14-21, iteration loop with periodic residual check, six-load-case bookkeeping).
+// All arithmetic of the method runs in the kernels of dr_kernels_*.cuh; there is no CPU fallback.
+#include <cuda_runtime.h>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <algorithm>
+
+#include "../../include/dr.h"
+#include "dr_layout.cuh"
+#include "dr_kernels_aux.cuh"
+#include "dr_kernels_split.cuh"
+#include "dr_kernels_fused.cuh"
+
+#define FUSED_TX 32
+#define FUSED_TY 16
+
+struct dr_handle {
+    DrLayout L;
+    double h;
+    cudaStream_t st;
+    // workspace carving (device)
+    double* buf[2][F_COUNT];
+    double *K0, *G0, *K, *G;
+    double* partial;            // DR_AVG_BLOCKS * 6
+    double* avg_dev;            // 6
+    unsigned long long* res_bits;
+    unsigned long long* hmax_bits;
+    unsigned int* flags;
+    // host
+    double* pinned;             // 8 doubles, page-locked
+    cudaEvent_t e0, e1;
+    // parameters
+    double cfl, st_factor, void_rel;
+    int ncheck, gavg, bc_mode, kernel;
+    double void_applied;        // void_rel currently baked into K,G
+    double hmax;
+    // state
+    int cur;                    // ping-pong buffer that holds the current fields
+    bool have_fields;
+    int cur_lc;
+    double cur_eps0;
+    // results
+    double Ccol[6][6];
+    bool have[6];
+    double avg[6];
+    bool have_avg;
+    int iters;
+    double residual, ms;
+    long long launches;
+    int fused_lz;
+    std::string err;
+};
+
+static dr_status fail(dr_handle* H, dr_status s, const std::string& msg) {
+    if (H) H->err = msg;
+    return s;
+}
+
+static bool cuda_ok(dr_handle* H, cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return true;
+    if (H) H->err = std::string(what) + ": " + cudaGetErrorString(e);
+    return false;
+}
+
+#define CK(call) do { if (!cuda_ok(H, (call), #call)) return DR_ERR_CUDA; } while (0)
+#define CKL(what) do { H->launches++; if (!cuda_ok(H, cudaGetLastError(), what)) return DR_ERR_CUDA; } while (0)
+
+static size_t align_up(size_t a, size_t m) { return (a + m - 1) / m * m; }
+
+static bool sizes_ok(int nx, int ny, int nz) {
+    return nx >= 2 && ny >= 2 && nz >= 2 && nx <= 8192 && ny <= 8192 && nz <= 8192;
+}
+
+static size_t field_bytes(const DrLayout& L) { return align_up((size_t)L.count * sizeof(double), 256); }
+static const int N_BIG = 2 * F_COUNT + 4;        // 18 state fields + K0, G0, K, G
+static const size_t SMALL_BYTES = align_up((size_t)DR_AVG_BLOCKS * 6 * sizeof(double), 256) + 1024;
+
+extern "C" size_t dr_workspace_bytes(int nx, int ny, int nz) {
+    if (!sizes_ok(nx, ny, nz)) return 0;
+    DrLayout L = dr_make_layout(nx, ny, nz);
+    return (size_t)N_BIG * field_bytes(L) + SMALL_BYTES;
+}
+
+// z-chunk length of the fused kernel: make the CTA count fill whole waves of 148 SMs while keeping the
+// priming overhead (one extra step per chunk) small
+static int choose_lz(const DrLayout& L) {
+    const int tiles = ((L.nx + 1 + FUSED_TX - 3) / (FUSED_TX - 2)) * ((L.ny + 1 + FUSED_TY - 3) / (FUSED_TY - 2));
+    const int layers = L.nz + 1;
+    int best_lz = layers;
+    double best = -1.0;
+    for (int c = 1; c <= 64 && c <= layers; ++c) {
+        int lz = (layers + c - 1) / c;
+        int chunks = (layers + lz - 1) / lz;
+        double blocks = (double)tiles * chunks;
+        double waves = std::ceil(blocks / 148.0);
+        double eff = blocks / (waves * 148.0) * (double)layers / ((double)chunks * (lz + 1));
+        if (eff > best + 1e-9) { best = eff; best_lz = lz; }
+    }
+    return best_lz;
+}
+
+extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K, const double* G,
+                               void* workspace, size_t workspace_bytes, void* cuda_stream, dr_handle** out) {
+    if (!out) return DR_ERR_ARG;
+    *out = nullptr;
+    if (!sizes_ok(nx, ny, nz) || !(h > 0.0) || !std::isfinite(h) || !K || !G) return DR_ERR_ARG;
+    if (!workspace || ((uintptr_t)workspace & 255u) || workspace_bytes < dr_workspace_bytes(nx, ny, nz)) return DR_ERR_WORKSPACE;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return DR_ERR_CUDA; }
+
+    dr_handle* H = new dr_handle();
+    H->L = dr_make_layout(nx, ny, nz);
+    H->h = h;
+    H->st = (cudaStream_t)cuda_stream;
+    const size_t fb = field_bytes(H->L);
+    char* p = (char*)workspace;
+    for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) { H->buf[b][f] = (double*)p; p += fb; }
+    H->K0 = (double*)p; p += fb; H->G0 = (double*)p; p += fb; H->K = (double*)p; p += fb; H->G = (double*)p; p += fb;
+    H->partial = (double*)p; p += align_up((size_t)DR_AVG_BLOCKS * 6 * sizeof(double), 256);
+    H->avg_dev = (double*)p; p += 256;
+    H->res_bits = (unsigned long long*)p; p += 256;
+    H->hmax_bits = (unsigned long long*)p; p += 256;
+    H->flags = (unsigned int*)p; p += 256;
+    H->pinned = nullptr; H->e0 = H->e1 = nullptr;
+    H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->kernel = 0;
+    H->void_applied = 0.0; H->hmax = 0.0;
+    H->cur = 0; H->have_fields = false; H->cur_lc = -1; H->cur_eps0 = 0.0;
+    for (int a = 0; a < 6; ++a) { H->have[a] = false; H->avg[a] = 0; for (int b = 0; b < 6; ++b) H->Ccol[a][b] = 0.0; }
+    H->have_avg = false; H->iters = 0; H->residual = 0.0; H->ms = 0.0; H->launches = 0;
+    H->fused_lz = choose_lz(H->L);
+
+    dr_status st = DR_OK;
+    do {
+        if (!cuda_ok(H, cudaMallocHost((void**)&H->pinned, 8 * sizeof(double)), "cudaMallocHost")) { st = DR_ERR_CUDA; break; }
+        if (!cuda_ok(H, cudaEventCreate(&H->e0), "cudaEventCreate") || !cuda_ok(H, cudaEventCreate(&H->e1), "cudaEventCreate")) { st = DR_ERR_CUDA; break; }
+        // state fields and moduli boxes start as zeros (halo nodes are never written afterwards)
+        if (!cuda_ok(H, cudaMemsetAsync(workspace, 0, (size_t)N_BIG * fb + SMALL_BYTES, H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }
+        dim3 blk(64, 4, 1), grd((nx + 2 + 63) / 64, (ny + 2 + 3) / 4, nz + 2);
+        k_pad_moduli<<<grd, blk, 0, H->st>>>(H->L, K, G, H->K0, H->G0, H->flags, H->hmax_bits);
+        H->launches++;
+        if (!cuda_ok(H, cudaGetLastError(), "k_pad_moduli")) { st = DR_ERR_CUDA; break; }
+        const long long cnt = H->L.count;
+        k_void_clamp<<<(unsigned)((cnt + 255) / 256), 256, 0, H->st>>>(H->L, H->K0, H->G0, H->K, H->G, 0.0);
+        H->launches++;
+        if (!cuda_ok(H, cudaGetLastError(), "k_void_clamp")) { st = DR_ERR_CUDA; break; }
+        unsigned long long hb = 0; unsigned int fl = 0;
+        if (!cuda_ok(H, cudaMemcpyAsync(&hb, H->hmax_bits, 8, cudaMemcpyDeviceToHost, H->st), "memcpy") ||
+            !cuda_ok(H, cudaMemcpyAsync(&fl, H->flags, 4, cudaMemcpyDeviceToHost, H->st), "memcpy") ||
+            !cuda_ok(H, cudaStreamSynchronize(H->st), "cudaStreamSynchronize")) { st = DR_ERR_CUDA; break; }
+        if (fl) { st = DR_ERR_ARG; break; }
+        std::memcpy(&H->hmax, &hb, 8);
+        // opt in to the large dynamic shared memory of the fused kernel (all instantiations)
+        const int smem = (int)DrFusedCfg<FUSED_TX, FUSED_TY>::SMEM;
+        cudaError_t e = cudaSuccess;
+        e = cudaFuncSetAttribute(k_pt_fused<0, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<0, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (!cuda_ok(H, e, "cudaFuncSetAttribute")) { st = DR_ERR_CUDA; break; }
+    } while (0);
+    if (st != DR_OK) {
+        if (H->pinned) cudaFreeHost(H->pinned);
+        if (H->e0) cudaEventDestroy(H->e0);
+        if (H->e1) cudaEventDestroy(H->e1);
+        delete H;
+        return st;
+    }
+    *out = H;
+    return DR_OK;
+}
+
+extern "C" dr_status dr_set_param(dr_handle* H, int id, double v) {
+    if (!H) return DR_ERR_ARG;
+    switch (id) {
+        case DR_CFL:       if (!(v > 0.0)) break; H->cfl = v; return DR_OK;
+        case DR_ST_FACTOR: if (!(v > 0.0)) break; H->st_factor = v; return DR_OK;
+        case DR_NCHECK:    if (!(v >= 1.0)) break; H->ncheck = (int)v; return DR_OK;
+        case DR_GAVG:      if (v != 0.0 && v != 1.0) break; H->gavg = (int)v; return DR_OK;
+        case DR_VOID_REL:  if (!(v >= 0.0)) break; H->void_rel = v; return DR_OK;
+        case DR_BC_MODE:   if (v != 0.0 && v != 1.0) break; H->bc_mode = (int)v; return DR_OK;
+        case DR_KERNEL:    if (v != 0.0 && v != 1.0) break; H->kernel = (int)v; return DR_OK;
+        default: break;
+    }
+    return fail(H, DR_ERR_ARG, "bad parameter id or value");
+}
+
+// Eq. 14-21, SURVEY O1 and O4
+static DrPT make_pt(const dr_handle* H, int lc, double eps0) {
+    DrPT P;
+    const DrLayout& L = H->L;
+    const int nmax = std::max(L.nx, std::max(L.ny, L.nz));
+    const double St = 2.0 * M_PI * std::sqrt(3.0) * H->st_factor;        // St_opt in 3-D
+    P.theta = H->cfl * St / nmax;                                         // dt~/Dt, from Eq. 14 and 16
+    P.rinv = 1.0 / (1.0 + P.theta);
+    P.c2t = H->cfl * H->cfl * H->h * H->h / P.theta;                      // Eq. 17
+    P.h = H->h; P.inv_h = 1.0 / H->h;
+    for (int a = 0; a < 9; ++a) P.D[a] = 0.0;
+    static const int slot[6] = {0, 4, 8, 5, 2, 1};                        // Dxx Dyy Dzz Dyz Dxz Dxy
+    P.D[slot[lc]] = eps0;
+    P.Lx = L.nx * H->h; P.Ly = L.ny * H->h; P.Lz = L.nz * H->h;
+    P.res_scale = H->h / std::fabs(eps0);
+    P.ghost_yz = (H->bc_mode == 1 || lc == 3);
+    P.ghost_xz = (H->bc_mode == 1 || lc == 4);
+    P.ghost_xy = (H->bc_mode == 1 || lc == 5);
+    return P;
+}
+
+static DrFields fields_of(dr_handle* H, int b) {
+    DrFields F; for (int f = 0; f < F_COUNT; ++f) F.f[f] = H->buf[b][f]; return F;
+}
+static DrConstFields cfields_of(dr_handle* H, int b) {
+    DrConstFields F; for (int f = 0; f < F_COUNT; ++f) F.f[f] = H->buf[b][f]; return F;
+}
+
+static dr_status prepare(dr_handle* H, int lc, double eps0) {
+    const DrLayout& L = H->L;
+    if (H->void_applied != H->void_rel) {
+        k_void_clamp<<<(unsigned)((L.count + 255) / 256), 256, 0, H->st>>>(H->L, H->K0, H->G0, H->K, H->G, H->void_rel * H->hmax);
+        CKL("k_void_clamp");
+        H->void_applied = H->void_rel;
+    }
+    DrPT P = make_pt(H, lc, eps0);
+    dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
+    if (H->gavg) k_bc_init<1><<<grd, blk, 0, H->st>>>(H->L, P, fields_of(H, 0), H->K, H->G);
+    else         k_bc_init<0><<<grd, blk, 0, H->st>>>(H->L, P, fields_of(H, 0), H->K, H->G);
+    CKL("k_bc_init");
+    H->cur = 0; H->have_fields = true; H->cur_lc = lc; H->cur_eps0 = eps0;
+    return DR_OK;
+}
+
+// one PT iteration; with_res: also accumulate the residual max-norm into res_bits (caller zeroes it)
+static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
+    const DrLayout& L = H->L;
+    if (H->kernel == 1) {
+        dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
+        DrFields F = fields_of(H, H->cur);
+        if (H->gavg) k_stress_split<1><<<grd, blk, 0, H->st>>>(H->L, P, F, H->K, H->G);
+        else         k_stress_split<0><<<grd, blk, 0, H->st>>>(H->L, P, F, H->K, H->G);
+        CKL("k_stress_split");
+        dim3 grv((L.nx + 63) / 64, (L.ny + 3) / 4, L.nz);
+        if (H->gavg) { if (with_res) k_velocity_split<1, 1><<<grv, blk, 0, H->st>>>(H->L, P, F, H->K, H->G, H->res_bits);
+                       else          k_velocity_split<1, 0><<<grv, blk, 0, H->st>>>(H->L, P, F, H->K, H->G, H->res_bits); }
+        else         { if (with_res) k_velocity_split<0, 1><<<grv, blk, 0, H->st>>>(H->L, P, F, H->K, H->G, H->res_bits);
+                       else          k_velocity_split<0, 0><<<grv, blk, 0, H->st>>>(H->L, P, F, H->K, H->G, H->res_bits); }
+        CKL("k_velocity_split");
+        return DR_OK;
+    }
+    const int lz = H->fused_lz;
+    dim3 blk(FUSED_TX, FUSED_TY, 1);
+    dim3 grd((L.nx + 1 + FUSED_TX - 3) / (FUSED_TX - 2), (L.ny + 1 + FUSED_TY - 3) / (FUSED_TY - 2), (L.nz + 1 + lz - 1) / lz);
+    const size_t smem = DrFusedCfg<FUSED_TX, FUSED_TY>::SMEM;
+    DrConstFields A = cfields_of(H, H->cur);
+    DrFields B = fields_of(H, H->cur ^ 1);
+    if (H->gavg) { if (with_res) k_pt_fused<1, 1, FUSED_TX, FUSED_TY><<<grd, blk, smem, H->st>>>(H->L, P, A, B, H->K, H->G, lz, H->res_bits);
+                   else          k_pt_fused<1, 0, FUSED_TX, FUSED_TY><<<grd, blk, smem, H->st>>>(H->L, P, A, B, H->K, H->G, lz, H->res_bits); }
+    else         { if (with_res) k_pt_fused<0, 1, FUSED_TX, FUSED_TY><<<grd, blk, smem, H->st>>>(H->L, P, A, B, H->K, H->G, lz, H->res_bits);
+                   else          k_pt_fused<0, 0, FUSED_TX, FUSED_TY><<<grd, blk, smem, H->st>>>(H->L, P, A, B, H->K, H->G, lz, H->res_bits); }
+    CKL("k_pt_fused");
+    H->cur ^= 1;
+    return DR_OK;
+}
+
+static dr_status read_residual(dr_handle* H, double* r) {
+    CK(cudaMemcpyAsync(H->pinned, H->res_bits, 8, cudaMemcpyDeviceToHost, H->st));
+    CK(cudaStreamSynchronize(H->st));
+    std::memcpy(r, H->pinned, 8);
+    return DR_OK;
+}
+
+static dr_status averages(dr_handle* H, int lc, double eps0) {
+    const DrLayout& L = H->L;
+    k_avg_partial<<<DR_AVG_BLOCKS, DR_AVG_THREADS, 0, H->st>>>(H->L, cfields_of(H, H->cur), H->partial);
+    CKL("k_avg_partial");
+    k_avg_final<<<1, 256, 0, H->st>>>(H->partial, DR_AVG_BLOCKS, 1.0 / ((double)L.nx * L.ny * L.nz), H->avg_dev);
+    CKL("k_avg_final");
+    CK(cudaMemcpyAsync(H->pinned, H->avg_dev, 6 * sizeof(double), cudaMemcpyDeviceToHost, H->st));
+    CK(cudaEventRecord(H->e1, H->st));
+    CK(cudaStreamSynchronize(H->st));
+    for (int m = 0; m < 6; ++m) { H->avg[m] = H->pinned[m]; H->Ccol[lc][m] = H->avg[m] / eps0; }   // Eq. 9, 22
+    H->have_avg = true; H->have[lc] = true;
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, H->e0, H->e1));
+    H->ms = ms;
+    return DR_OK;
+}
+
+static bool bad_lc(dr_handle* H, int lc, double eps0) {
+    if (lc < 0 || lc > 5 || !(eps0 != 0.0) || !std::isfinite(eps0)) { H->err = "bad load case or eps0"; return true; }
+    return false;
+}
+
+extern "C" dr_status dr_solve(dr_handle* H, int lc, double eps0, double tol, int maxiter) {
+    if (!H) return DR_ERR_ARG;
+    if (bad_lc(H, lc, eps0)) return DR_ERR_ARG;
+    if (!(tol > 0.0) || maxiter < 1) return fail(H, DR_ERR_ARG, "bad tol or maxiter");
+    CK(cudaEventRecord(H->e0, H->st));
+    dr_status s = prepare(H, lc, eps0);
+    if (s != DR_OK) return s;
+    const DrPT P = make_pt(H, lc, eps0);
+    dr_status status = DR_MAXITER;
+    H->residual = INFINITY;
+    int it;
+    for (it = 1; it <= maxiter; ++it) {
+        const bool chk = (it % H->ncheck == 0);
+        if (chk) CK(cudaMemsetAsync(H->res_bits, 0, 8, H->st));
+        s = iteration(H, P, chk);
+        if (s != DR_OK) return s;
+        if (chk) {
+            double r;
+            s = read_residual(H, &r);
+            if (s != DR_OK) return s;
+            H->residual = r;
+            if (!std::isfinite(r)) { status = DR_ERR_DIVERGED; break; }
+            if (r <= tol) { status = DR_OK; break; }
+        }
+    }
+    H->iters = std::min(it, maxiter);
+    if (status == DR_ERR_DIVERGED) {
+        CK(cudaEventRecord(H->e1, H->st));
+        CK(cudaStreamSynchronize(H->st));
+        return fail(H, status, "residual is not finite");
+    }
+    s = averages(H, lc, eps0);
+    if (s != DR_OK) return s;
+    if (status == DR_MAXITER) H->err = "maxiter reached";
+    return status;
+}
+
+extern "C" dr_status dr_step(dr_handle* H, int lc, double eps0, int niter) {
+    if (!H) return DR_ERR_ARG;
+    if (bad_lc(H, lc, eps0)) return DR_ERR_ARG;
+    if (niter < 0) return fail(H, DR_ERR_ARG, "bad niter");
+    CK(cudaEventRecord(H->e0, H->st));
+    dr_status s = prepare(H, lc, eps0);
+    if (s != DR_OK) return s;
+    const DrPT P = make_pt(H, lc, eps0);
+    double r = 0.0;
+    for (int it = 1; it <= niter; ++it) {
+        const bool last = (it == niter);
+        if (last) CK(cudaMemsetAsync(H->res_bits, 0, 8, H->st));
+        s = iteration(H, P, last);
+        if (s != DR_OK) return s;
+    }
+    if (niter > 0) { s = read_residual(H, &r); if (s != DR_OK) return s; }
+    H->iters = niter; H->residual = r;
+    return averages(H, lc, eps0);
+}
+
+extern "C" dr_status dr_iterate(dr_handle* H, int lc, double eps0, int niter) {
+    if (!H) return DR_ERR_ARG;
+    if (bad_lc(H, lc, eps0)) return DR_ERR_ARG;
+    if (niter < 0) return fail(H, DR_ERR_ARG, "bad niter");
+    if (!H->have_fields || lc != H->cur_lc || eps0 != H->cur_eps0)
+        return fail(H, DR_ERR_STATE, "dr_iterate needs a previous dr_step/dr_solve with the same load case and eps0");
+    const DrPT P = make_pt(H, lc, eps0);
+    for (int it = 0; it < niter; ++it) {
+        dr_status s = iteration(H, P, false);
+        if (s != DR_OK) return s;
+    }
+    return DR_OK;
+}
+
+extern "C" dr_status dr_effective_C(dr_handle* H, double out[36]) {
+    if (!H || !out) return DR_ERR_ARG;
+    for (int lc = 0; lc < 6; ++lc) if (!H->have[lc]) return fail(H, DR_ERR_STATE, "not all six load cases solved");
+    for (int m = 0; m < 6; ++m) for (int lc = 0; lc < 6; ++lc) out[6 * m + lc] = H->Ccol[lc][m];
+    return DR_OK;
+}
+
+extern "C" dr_status dr_avg_stress(dr_handle* H, double out[6]) {
+    if (!H || !out) return DR_ERR_ARG;
+    if (!H->have_avg) return fail(H, DR_ERR_STATE, "no solve yet");
+    for (int m = 0; m < 6; ++m) out[m] = H->avg[m];
+    return DR_OK;
+}
+
+extern "C" dr_status dr_info(dr_handle* H, int* iters, double* residual, double* ms) {
+    if (!H) return DR_ERR_ARG;
+    if (iters) *iters = H->iters;
+    if (residual) *residual = H->residual;
+    if (ms) *ms = H->ms;
+    return DR_OK;
+}
+
+extern "C" dr_status dr_get_field(dr_handle* H, int field, double* dst, size_t n) {
+    if (!H || !dst) return DR_ERR_ARG;
+    if (field < 0 || field >= F_COUNT) return fail(H, DR_ERR_ARG, "bad field id");
+    if (!H->have_fields) return fail(H, DR_ERR_STATE, "no fields yet");
+    const DrLayout& L = H->L;
+    int ex = L.nx, ey = L.ny, ez = L.nz;
+    switch (field) {
+        case F_VX: ex++; break; case F_VY: ey++; break; case F_VZ: ez++; break;
+        case F_TYZ: ey++; ez++; break; case F_TXZ: ex++; ez++; break; case F_TXY: ex++; ey++; break;
+        default: break;
+    }
+    if (n != (size_t)ex * ey * ez) return fail(H, DR_ERR_ARG, "bad field size");
+    dim3 blk(64, 4, 1), grd((ex + 63) / 64, (ey + 3) / 4, ez);
+    k_export<<<grd, blk, 0, H->st>>>(H->L, H->buf[H->cur][field], dst, ex, ey, ez);
+    CKL("k_export");
+    CK(cudaStreamSynchronize(H->st));
+    return DR_OK;
+}
+
+extern "C" dr_status dr_solve_image_host(int nx, int ny, int nz, double h, const double* K_host, const double* G_host,
+                                         double* stage_device, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                                         double eps0, double tol, int maxiter, int ncheck, double C_out[36], int iters_out[6]) {
+    if (!sizes_ok(nx, ny, nz) || !K_host || !G_host || !stage_device || !C_out) return DR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t N = (size_t)nx * ny * nz;
+    if (cudaMemcpyAsync(stage_device, K_host, N * sizeof(double), cudaMemcpyHostToDevice, st) != cudaSuccess) return DR_ERR_CUDA;
+    if (cudaMemcpyAsync(stage_device + N, G_host, N * sizeof(double), cudaMemcpyHostToDevice, st) != cudaSuccess) return DR_ERR_CUDA;
+    dr_handle* H = nullptr;
+    dr_status s = dr_create(nx, ny, nz, h, stage_device, stage_device + N, workspace, workspace_bytes, cuda_stream, &H);
+    if (s != DR_OK) return s;
+    dr_status worst = DR_OK;
+    if (ncheck > 0) dr_set_param(H, DR_NCHECK, ncheck);
+    for (int lc = 0; lc < 6; ++lc) {
+        s = dr_solve(H, lc, eps0, tol, maxiter);
+        if (iters_out) iters_out[lc] = H->iters;
+        if (s != DR_OK && s != DR_MAXITER) { dr_destroy(H); return s; }
+        if (s == DR_MAXITER) worst = DR_MAXITER;
+    }
+    s = dr_effective_C(H, C_out);
+    dr_destroy(H);
+    return s != DR_OK ? s : worst;
+}
+
+extern "C" long long dr_launch_count(dr_handle* H) { return H ? H->launches : 0; }
+
+extern "C" const char* dr_last_error(dr_handle* H) { return H ? H->err.c_str() : "null handle"; }
+
+extern "C" void dr_destroy(dr_handle* H) {
+    if (!H) return;
+    cudaStreamSynchronize(H->st);
+    if (H->pinned) cudaFreeHost(H->pinned);
+    if (H->e0) cudaEventDestroy(H->e0);
+    if (H->e1) cudaEventDestroy(H->e1);
+    delete H;
+}

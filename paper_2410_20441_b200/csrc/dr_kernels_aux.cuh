@@ -1,0 +1,191 @@
+// dr_kernels_aux.cuh -- set-up, boundary/initial fields, reductions and field export kernels of libdr.
+// (SURVEY 8(a) rows a0, a4, a5 helper, a6.)  P:NNN = PAPER.md line.
+#pragma once
+#include "dr_layout.cuh"
+
+// ------------------------------------------------------------------------------------------------------
+// shear modulus on an edge from the four cells round it (Reading R4): harmonic mean, 0 if any is 0
+// (1/0 = +inf and 4/inf = 0 in IEEE arithmetic, so no branch is needed); GAVG=1: arithmetic mean.
+template <int GAVG>
+__device__ __forceinline__ double dr_edge_mean(double a, double b, double c, double d) {
+    if (GAVG) return 0.25 * (a + b + c + d);
+    return 4.0 / (1.0 / a + 1.0 / b + 1.0 / c + 1.0 / d);
+}
+
+__device__ __forceinline__ double dr_u0(const DrPT& P, int a, double x, double y, double z) {
+    return P.D[3 * a] * x + P.D[3 * a + 1] * y + P.D[3 * a + 2] * z;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// a0: copy the caller's dense K,G into the padded box with a replicate halo; validate; max of K+4G/3.
+// flags[0] |= 1 if any modulus is negative or not finite.  hmax_bits: atomicMax on the bit pattern.
+__global__ void k_pad_moduli(DrLayout L, const double* __restrict__ Ksrc, const double* __restrict__ Gsrc,
+                             double* __restrict__ Kp, double* __restrict__ Gp,
+                             unsigned int* flags, unsigned long long* hmax_bits) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x - 1;      // -1 .. nx
+    int j = blockIdx.y * blockDim.y + threadIdx.y - 1;      // -1 .. ny
+    int k = blockIdx.z - 1;                                  // -1 .. nz
+    if (i > L.nx || j > L.ny) return;
+    int ci = min(max(i, 0), L.nx - 1), cj = min(max(j, 0), L.ny - 1), ck = min(max(k, 0), L.nz - 1);
+    size_t s = (size_t)ci + (size_t)L.nx * ((size_t)cj + (size_t)L.ny * ck);
+    double Kv = Ksrc[s], Gv = Gsrc[s];
+    long long q = L.origin + i + L.sy * j + L.sz * k;
+    Kp[q] = Kv; Gp[q] = Gv;
+    if (i == ci && j == cj && k == ck) {
+        bool bad = !(Kv >= 0.0) || !(Gv >= 0.0) || isinf(Kv) || isinf(Gv);
+        if (bad) atomicOr(flags, 1u);
+        else {
+            double Hc = Kv + 4.0 * Gv / 3.0;
+            unsigned long long b = (unsigned long long)__double_as_longlong(Hc);
+            // cheap pre-filter, then atomic
+            if (b > *((volatile unsigned long long*)hmax_bits)) atomicMax(hmax_bits, b);
+        }
+    }
+}
+
+// optional void clamp (Reading R9): K = G = 0 where K0+4G0/3 <= thr, else the original values (halo included)
+__global__ void k_void_clamp(DrLayout L, const double* __restrict__ K0, const double* __restrict__ G0,
+                             double* __restrict__ Kp, double* __restrict__ Gp, double thr) {
+    long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= L.count) return;
+    double Kv = K0[q], Gv = G0[q];
+    if (thr > 0.0 && Kv + 4.0 * Gv / 3.0 <= thr) { Kv = 0.0; Gv = 0.0; }
+    Kp[q] = Kv; Gp[q] = Gv;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// a4: initial fields and boundary values (Reading R8): every velocity node := affine u0 at its
+// own position, stresses := Hooke's law of the uniform strain (boundary shear zero where the face is free-slip,
+// App. A.1).  One thread per node of the (nx+1)(ny+1)(nz+1) box.
+template <int GAVG>
+__global__ void k_bc_init(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, const double* __restrict__ Gp) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int j = blockIdx.y * blockDim.y + threadIdx.y;
+    int k = blockIdx.z;
+    if (i > L.nx || j > L.ny) return;
+    const int nx = L.nx, ny = L.ny, nz = L.nz;
+    const long long sy = L.sy, sz = L.sz;
+    long long q = L.origin + i + sy * j + sz * k;
+    const double h = P.h;
+    const double Exx = P.D[0], Eyy = P.D[4], Ezz = P.D[8];
+    const double gyz = P.D[5] + P.D[7], gxz = P.D[2] + P.D[6], gxy = P.D[1] + P.D[3];
+    const double trE = Exx + Eyy + Ezz;
+    const bool ci = i < nx, cj = j < ny, ck = k < nz;
+    F.f[F_VX][q] = (cj && ck) ? dr_u0(P, 0, i * h, (j + 0.5) * h, (k + 0.5) * h) : 0.0;
+    F.f[F_VY][q] = (ci && ck) ? dr_u0(P, 1, (i + 0.5) * h, j * h, (k + 0.5) * h) : 0.0;
+    F.f[F_VZ][q] = (ci && cj) ? dr_u0(P, 2, (i + 0.5) * h, (j + 0.5) * h, k * h) : 0.0;
+    double sxx = 0, syy = 0, szz = 0;
+    if (ci && cj && ck) {
+        double Kc = Kp[q], Gc = Gp[q];
+        double pr = -Kc * trE;
+        sxx = -pr + 2.0 * Gc * (Exx - trE / 3.0);
+        syy = -pr + 2.0 * Gc * (Eyy - trE / 3.0);
+        szz = -pr + 2.0 * Gc * (Ezz - trE / 3.0);
+    }
+    F.f[F_SXX][q] = sxx; F.f[F_SYY][q] = syy; F.f[F_SZZ][q] = szz;
+    double txy = 0, txz = 0, tyz = 0;
+    const bool bi = (i == 0 || i == nx), bj = (j == 0 || j == ny), bk = (k == 0 || k == nz);
+    if (ck && (!(bi || bj) || P.ghost_xy))
+        txy = dr_edge_mean<GAVG>(Gp[q - 1 - sy], Gp[q - sy], Gp[q - 1], Gp[q]) * gxy;
+    if (cj && (!(bi || bk) || P.ghost_xz))
+        txz = dr_edge_mean<GAVG>(Gp[q - 1 - sz], Gp[q - sz], Gp[q - 1], Gp[q]) * gxz;
+    if (ci && (!(bj || bk) || P.ghost_yz))
+        tyz = dr_edge_mean<GAVG>(Gp[q - sy - sz], Gp[q - sz], Gp[q - sy], Gp[q]) * gyz;
+    F.f[F_TXY][q] = txy; F.f[F_TXZ][q] = txz; F.f[F_TYZ][q] = tyz;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// block-wide reductions: warp shuffles, then one shared-memory pass (BASELINE north_star (b)).
+// max over the bit patterns of non-negative doubles: order-preserving as unsigned integers, and a NaN
+// (pattern above +inf) wins, so divergence is never hidden.
+__device__ __forceinline__ unsigned long long dr_warp_max_bits(unsigned long long v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        unsigned long long w = __shfl_xor_sync(0xffffffffu, v, o);
+        v = w > v ? w : v;
+    }
+    return v;
+}
+
+// all threads of the block must call; result valid in thread 0
+__device__ __forceinline__ unsigned long long dr_block_max_bits(unsigned long long v, unsigned long long* smem32) {
+    const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int nthr = blockDim.x * blockDim.y * blockDim.z;
+    v = dr_warp_max_bits(v);
+    if ((tid & 31) == 0) smem32[tid >> 5] = v;
+    __syncthreads();
+    if (tid < 32) {
+        v = (tid < (nthr + 31) / 32) ? smem32[tid] : 0ull;
+        v = dr_warp_max_bits(v);
+    }
+    return v;
+}
+
+__device__ __forceinline__ double dr_warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// a6: volume averages (Eq. 7; Reading R7).  Each block walks whole x-rows (j,k) of the node box in a
+// fixed order and writes 6 partial sums; k_avg_final adds the partials in a fixed order -> run-to-run
+// deterministic.  Normal stresses: plain cell sum; edge shears: trapezoid weights 1/2 on the first/last index.
+#define DR_AVG_BLOCKS 1184      // 8 x 148 SMs
+#define DR_AVG_THREADS 256
+__global__ void __launch_bounds__(DR_AVG_THREADS)
+k_avg_partial(DrLayout L, DrConstFields F, double* __restrict__ partial) {
+    const int nx = L.nx, ny = L.ny, nz = L.nz;
+    const long long rows = (long long)(ny + 1) * (nz + 1);
+    double s[6] = {0, 0, 0, 0, 0, 0};
+    for (long long r = blockIdx.x; r < rows; r += gridDim.x) {
+        int j = (int)(r % (ny + 1)), k = (int)(r / (ny + 1));
+        const bool cj = j < ny, ck = k < nz;
+        const double wj = (j == 0 || j == ny) ? 0.5 : 1.0, wk = (k == 0 || k == nz) ? 0.5 : 1.0;
+        long long q0 = L.origin + L.sy * j + L.sz * k;
+        for (int i = threadIdx.x; i <= nx; i += blockDim.x) {
+            long long q = q0 + i;
+            const bool ci = i < nx;
+            const double wi = (i == 0 || i == nx) ? 0.5 : 1.0;
+            if (ci && cj && ck) { s[0] += F.f[F_SXX][q]; s[1] += F.f[F_SYY][q]; s[2] += F.f[F_SZZ][q]; }
+            if (ci) s[3] += wj * wk * F.f[F_TYZ][q];
+            if (cj) s[4] += wi * wk * F.f[F_TXZ][q];
+            if (ck) s[5] += wi * wj * F.f[F_TXY][q];
+        }
+    }
+    __shared__ double sm[6][DR_AVG_THREADS / 32];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+        double v = dr_warp_sum(s[m]);
+        if ((threadIdx.x & 31) == 0) sm[m][threadIdx.x >> 5] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        double v = 0;
+        for (int w = 0; w < DR_AVG_THREADS / 32; ++w) v += sm[threadIdx.x][w];
+        partial[(size_t)blockIdx.x * 6 + threadIdx.x] = v;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_avg_final(const double* __restrict__ partial, int nblocks, double invN, double* out6) {
+    __shared__ double sm[6][256];
+    double s[6] = {0, 0, 0, 0, 0, 0};
+    for (int b = threadIdx.x; b < nblocks; b += 256)
+        for (int m = 0; m < 6; ++m) s[m] += partial[(size_t)b * 6 + m];
+    for (int m = 0; m < 6; ++m) sm[m][threadIdx.x] = s[m];
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) for (int m = 0; m < 6; ++m) sm[m][threadIdx.x] += sm[m][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x < 6) out6[threadIdx.x] = sm[threadIdx.x][0] * invN;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// export one field from the padded box to a dense array of its logical shape (dr_get_field)
+__global__ void k_export(DrLayout L, const double* __restrict__ src, double* __restrict__ dst, int ex, int ey, int ez) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int j = blockIdx.y * blockDim.y + threadIdx.y;
+    int k = blockIdx.z;
+    if (i >= ex || j >= ey || k >= ez) return;
+    dst[(size_t)i + (size_t)ex * ((size_t)j + (size_t)ey * k)] = src[L.origin + i + L.sy * j + L.sz * k];
+}

@@ -1,0 +1,187 @@
+"""GPU parity: libdr (through the C ABI) against the CPU oracle on the same seeded inputs.
+Bars (BASELINE.json north_star): per-field relative L-inf <= 1e-10 after a fixed iteration count,
+C_ij relative <= 1e-6 at convergence."""
+import numpy as np
+import pytest
+
+from paper_2410_20441_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FIELD_TOL = 1e-10
+C_TOL = 1e-6
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2410_20441_b200 import binding
+    binding.lib()
+    return binding
+
+
+def to_dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def field_errors(o, s, K, G, eps0, h=1.0):
+    """err_f = |f_gpu - f_cpu|_inf / max(|f_cpu|_inf, 1e-6 S); S = eps0 L (velocities), max(K+4G/3) eps0 (stresses)"""
+    L = h * max(K.shape)
+    Sv = abs(eps0) * L
+    Ss = abs(eps0) * float(np.max(K + 4 * G / 3))
+    errs = []
+    for f in range(9):
+        a = o.get_field(f)
+        b = s.get_field(f).cpu().numpy()
+        assert a.shape == b.shape
+        S = Sv if f < 3 else Ss
+        errs.append(float(np.max(np.abs(a - b)) / max(np.max(np.abs(a)), 1e-6 * S)))
+    return errs
+
+
+def run_pair(oracle_mod, gpu, K, G, lc, eps0, niter, h=1.0, **params):
+    o = oracle_mod.Oracle(K, G, h=h, **{k: v for k, v in params.items() if k != "kernel"})
+    s = gpu.Solver(to_dev(K), to_dev(G), h=h, **params)
+    o.step(lc, eps0, niter)
+    s.step(lc, eps0, niter)
+    errs = field_errors(o, s, K, G, eps0, h)
+    ro, rs = o.info()[1], s.info()[1]
+    ao, as_ = o.avg_stress(), s.avg_stress()
+    return errs, ro, rs, ao, as_
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("lc", range(6))
+def test_fields_config1_sphere_100_iterations(oracle_mod, gpu, kernel, lc):
+    K, G, _ = inputs.config1_sphere()
+    errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, 1e-4, 100, kernel=kernel)
+    assert max(errs) <= FIELD_TOL, errs
+    assert abs(ro - rs) <= 1e-9 * ro
+    assert np.max(np.abs(ao - as_)) <= 1e-10 * np.max(np.abs(ao))
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("shape,h", [((37, 21, 19), 0.5), ((5, 64, 7), 1.0), ((2, 2, 2), 2.0), ((61, 29, 33), 1.0)])
+def test_fields_ragged_noncubic_random_moduli(oracle_mod, gpu, kernel, shape, h):
+    """several tiles with ragged tails in x, y and z; every voxel has different moduli"""
+    K, G = inputs.random_smooth(shape, seed=sum(shape))
+    for lc in (0, 3, 4, 5):
+        errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, -2e-3, 25, h=h, kernel=kernel)
+        assert max(errs) <= FIELD_TOL, (lc, errs)
+        assert abs(ro - rs) <= 1e-9 * ro
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_fields_void_and_fluid_cells(oracle_mod, gpu, kernel):
+    """degenerate moduli: exact void (K=G=0), fluid (G=0), 1e-6 contrast"""
+    K, G, m = inputs.random_two_phase((40, 33, 20), frac=0.3, seed=4, matrix=(37.0, 44.0), incl=(2.2, 0.0))
+    K[3:6, 10:20, 5:30] = 0.0
+    G[3:6, 10:20, 5:30] = 0.0
+    for lc in (1, 2, 4):
+        errs, ro, rs, _, _ = run_pair(oracle_mod, gpu, K, G, lc, 1e-4, 30, kernel=kernel)
+        assert max(errs) <= FIELD_TOL, (lc, errs)
+        assert np.isfinite(rs) and abs(ro - rs) <= 1e-9 * ro
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("params", [dict(bc_mode=1), dict(gavg=1), dict(cfl=0.5, st_factor=0.7), dict(void_rel=1e-5)])
+def test_fields_parameter_variants(oracle_mod, gpu, kernel, params):
+    K, G, _ = inputs.config1_sphere(n=24, r=4.0)
+    for lc in (0, 5):
+        errs, ro, rs, _, _ = run_pair(oracle_mod, gpu, K, G, lc, 1e-4, 40, kernel=kernel, **params)
+        assert max(errs) <= FIELD_TOL, (params, lc, errs)
+
+
+def test_zero_iterations_is_the_initial_field(oracle_mod, gpu):
+    K, G = inputs.random_smooth((9, 8, 7), seed=1)
+    for lc in range(6):
+        errs, _, _, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, 1e-3, 0, h=0.3)
+        assert max(errs) <= 1e-14, errs
+        assert np.max(np.abs(ao - as_)) <= 1e-13 * np.max(np.abs(ao))
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_converged_C_config1(oracle_mod, gpu, kernel):
+    """cfg 1 to tol 1e-8, same ncheck on both sides -> same iteration counts; C within 1e-6"""
+    K, G, _ = inputs.config1_sphere()
+    o = oracle_mod.Oracle(K, G)
+    Co, logo = o.solve_all(1e-4, 1e-8, 3200)
+    s = gpu.Solver(to_dev(K), to_dev(G), kernel=kernel)
+    Cs, logs = s.solve_all(1e-4, 1e-8, 3200)
+    assert [l[1] for l in logo] == [l[1] for l in logs]
+    assert all(l[0] == 0 for l in logs)
+    assert np.max(np.abs(Co - Cs)) <= C_TOL * np.max(np.abs(Co))
+    for lo, ls in zip(logo, logs):
+        assert abs(lo[2] - ls[2]) <= 1e-6 * lo[2]
+
+
+def test_converged_C_two_phase_48(oracle_mod, gpu):
+    K, G, _ = inputs.config4_grf(n=48, ell=6.0, seed=5)
+    o = oracle_mod.Oracle(K, G, ncheck=100)
+    Co, logo = o.solve_all(1e-4, 1e-8, 4800)
+    s = gpu.Solver(to_dev(K), to_dev(G), ncheck=100)
+    Cs, logs = s.solve_all(1e-4, 1e-8, 4800)
+    assert [l[1] for l in logo] == [l[1] for l in logs]
+    assert np.max(np.abs(Co - Cs)) <= C_TOL * np.max(np.abs(Co))
+
+
+def test_host_api_end_to_end(oracle_mod, gpu):
+    K, G, _ = inputs.config1_sphere(n=20, r=3.0)
+    C, iters, st = gpu.solve_image_host(K, G, tol=1e-8, maxiter=2000, ncheck=50)
+    o = oracle_mod.Oracle(K, G)
+    Co, logo = o.solve_all(1e-4, 1e-8, 2000)
+    assert st == 0 and iters == [l[1] for l in logo]
+    assert np.max(np.abs(Co - C)) <= C_TOL * np.max(np.abs(Co))
+
+
+def test_status_codes_and_errors(gpu):
+    import torch
+    K, G = inputs.homogeneous(8)
+    s = gpu.Solver(to_dev(K), to_dev(G))
+    with pytest.raises(gpu.DrError) as e:
+        s.effective_C()
+    assert e.value.status == gpu.ERR_STATE
+    with pytest.raises(gpu.DrError):
+        s.solve(7)
+    with pytest.raises(gpu.DrError):
+        s.solve(0, eps0=0.0)
+    with pytest.raises(gpu.DrError):
+        s.iterate(0, 1e-4, 3)                      # no fields yet
+    assert s.solve(0, 1e-4, 1e-30, 7) == gpu.MAXITER
+    assert s.info()[0] == 7
+    Kb = K.copy(); Kb[1, 2, 3] = -1.0
+    with pytest.raises(gpu.DrError) as e:
+        gpu.Solver(to_dev(Kb), to_dev(G))
+    assert e.value.status == gpu.ERR_ARG
+    Kb[1, 2, 3] = np.nan
+    with pytest.raises(gpu.DrError):
+        gpu.Solver(to_dev(Kb), to_dev(G))
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(gpu.DrError) as e:
+        gpu.Solver(to_dev(K), to_dev(G), workspace=small)
+    assert e.value.status == gpu.ERR_WORKSPACE
+
+
+def test_homogeneous_block_on_gpu(gpu):
+    K, G = inputs.homogeneous((33, 17, 40), 70.2, 29.0)
+    s = gpu.Solver(to_dev(K), to_dev(G), ncheck=10)
+    C, log = s.solve_all()
+    assert all(l[0] == 0 and l[1] == 10 and l[2] < 1e-11 for l in log), log
+    H = np.zeros((6, 6)); H[:3, :3] = 70.2 - 2 * 29 / 3
+    H[np.arange(3), np.arange(3)] = 70.2 + 4 * 29 / 3; H[np.arange(3, 6), np.arange(3, 6)] = 29.0
+    assert np.max(np.abs(C - H)) <= 1e-11 * 108.9
+
+
+def test_iterate_continues_step(oracle_mod, gpu):
+    K, G = inputs.random_smooth((20, 18, 16), seed=9)
+    o = oracle_mod.Oracle(K, G)
+    o.step(2, 1e-4, 30)
+    s = gpu.Solver(to_dev(K), to_dev(G))
+    s.step(2, 1e-4, 10)
+    s.iterate(2, 1e-4, 20)
+    import torch
+    torch.cuda.synchronize()
+    errs = field_errors(o, s, K, G, 1e-4)
+    assert max(errs) <= FIELD_TOL, errs
