@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fused pseudo-transient (PT) elasticity iteration of libdr on B200.
+
+Metric (BASELINE.json): PT voxel-updates/s, T_eff = 160 B x N x iterations / time against the measured HBM
+peak, and (with --time-to-solution) the time to the full 6x6 C_eff.
+
+A "step" is one PT iteration of the whole hot path as dr_solve runs it: the fused stress+velocity kernel
+(SURVEY 8(a) a2+a3) every step, the residual max-norm (a5) every `ncheck`-th step, and -- once per timed call --
+the initial/boundary fields (a4) and the volume averages -> C column (a6).  The timed region is ONE
+dr_solve(lc, eps0, tol=1e-300, maxiter=K) call, i.e. exactly K steps.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg2|cfg1|cfg5] [--time-to-solution]
+    python bench.py --impl reference ...      # the CPU oracle on the host cores (bounded sample)
+
+N > 1 (torchrun): the path shards over independent load cases -- rank r solves load case r mod 6 of the same
+image on its own GPU, no data-path collective ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2410_20441_b200 import inputs  # noqa: E402
+
+BYTES_PER_VOXEL_ITER = 160.0        # (2*9 + 2) fp64, SURVEY 8(d)
+WORKLOADS = {
+    "cfg1": dict(n=32, gen="config1_sphere", desc="32^3 centred spherical pore r=5, contrast 1e-6"),
+    "cfg2": dict(n=191, gen="config2_spheroid", desc="191^3 oblate fluid spheroid (40,40,8)"),
+    "cfg3": dict(n=191, gen="config3_random_spheres", desc="191^3 200 random spherical pores, contrast 1e-6"),
+    "cfg4": dict(n=479, gen="config4_grf", desc="479^3 thresholded Gaussian random field, 15% soft phase"),
+    "cfg5": dict(n=703, gen="config5_penny_cracks", desc="703^3 400 penny cracks, contrast 1e-6"),
+}
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (measured copy rate)"
+    except Exception:
+        return 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md; MEASURED_PEAKS.json absent)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            t = [x.strip() for x in r.split(",")]
+            if len(t) < 7:
+                continue
+            try:
+                sm.append(float(t[0])); mx.append(float(t[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, t[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_image(workload, n_override=None):
+    w = WORKLOADS[workload]
+    n = n_override or w["n"]
+    K, G, _ = getattr(inputs, w["gen"])(n=n)
+    return K, G, n
+
+
+def crop(K, G, m):
+    m = min(m, K.shape[0])
+    return np.ascontiguousarray(K[:m, :m, :m]), np.ascontiguousarray(G[:m, :m, :m]), m
+
+
+def oracle_rate(K, G, lc, eps0, sample_n, iters):
+    """time the oracle as it stands on the host cores: `iters` PT iterations on a sample_n^3 crop"""
+    from oracle import dro
+    Kc, Gc, m = crop(K, G, sample_n)
+    o = dro.Oracle(Kc, Gc)
+    o.step(lc, eps0, 1)
+    t0 = time.perf_counter()
+    o.iterate(lc, eps0, iters)
+    dt = time.perf_counter() - t0
+    return m ** 3 * iters / dt, dt, m
+
+
+def host_threads():
+    try:
+        return int(os.environ.get("OMP_NUM_THREADS", "")) if os.environ.get("OMP_NUM_THREADS") else len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    K, G, n = make_image(args.workload, args.n)
+    sample_n = min(n, args.cpu_sample_n)
+    from oracle import dro
+    Kc, Gc, m = crop(K, G, sample_n)
+    o = dro.Oracle(Kc, Gc)
+    o.step(args.lc, args.eps0, 0)
+    per = max(1, args.cpu_iters_per_step)
+    for _ in range(args.warmup):
+        o.iterate(args.lc, args.eps0, per)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.iterate(args.lc, args.eps0, per)
+    dt = time.perf_counter() - t0
+    rate = m ** 3 * per * args.steps / dt
+    sample = "%d^3 crop of %s, %d oracle PT iterations per step" % (m, args.workload, per)
+    line = {
+        "impl": "reference", "metric": "pt_voxel_updates_per_s", "value": rate, "unit": "voxel-updates/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s: %s" % (args.workload, WORKLOADS[args.workload]["desc"]), "load_case": args.lc},
+        "cpu_baseline": {"value": rate, "unit": "voxel-updates/s", "cores": host_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": "voxel-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="libdr", choices=["libdr", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
+    ap.add_argument("--n", type=int, default=None, help="override the grid size of the workload (debug)")
+    ap.add_argument("--lc", type=int, default=2)
+    ap.add_argument("--eps0", type=float, default=1e-4)
+    ap.add_argument("--ncheck", type=int, default=100)
+    ap.add_argument("--kernel", type=int, default=0, help="0 fused (default), 1 split baseline")
+    ap.add_argument("--cpu-sample-n", type=int, default=191)
+    ap.add_argument("--cpu-iters", type=int, default=100)
+    ap.add_argument("--cpu-iters-per-step", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-iters", type=int, default=50, help="PT iterations per load case in the host-buffer e2e call")
+    ap.add_argument("--time-to-solution", action="store_true", help="also solve all six load cases to tol 1e-8")
+    ap.add_argument("--tol", type=float, default=1e-8)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2410_20441_b200 import binding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libdr has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    K, G, n = make_image(args.workload, args.n)
+    N = n ** 3
+    Kd = torch.from_numpy(K).to(dev)
+    Gd = torch.from_numpy(G).to(dev)
+    lc = (args.lc + rank) % 6 if world > 1 else args.lc
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        s = binding.Solver(Kd, Gd, stream=stream, ncheck=args.ncheck, kernel=args.kernel)
+
+        def barrier():
+            torch.cuda.synchronize(dev)
+            if dist is not None:
+                dist.barrier()
+            torch.cuda.synchronize(dev)
+
+        # ---- warm-up, then the timed call: exactly K steps of the whole hot path
+        s.solve(lc, args.eps0, 1e-300, args.warmup)
+        barrier()
+        sampler = ClockSampler(local)
+        if rank == 0:
+            sampler.start()
+        l0 = s.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        s.solve(lc, args.eps0, 1e-300, args.steps)
+        e1.record(stream)
+        barrier()
+        launches = s.launch_count() - l0
+        ms = e0.elapsed_time(e1)
+        # ---- dominant kernel alone (k_pt_fused back to back, no residual): average launch duration
+        s.iterate(lc, args.eps0, 5)
+        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k0.record(stream)
+        s.iterate(lc, args.eps0, args.steps)
+        k1.record(stream)
+        torch.cuda.synchronize(dev)
+        kms = k0.elapsed_time(k1) / args.steps
+        clocks = sampler.stop() if rank == 0 else None
+        if dist is not None:
+            t = torch.tensor([ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+            dist.barrier()
+            dist.destroy_process_group()
+            dist = None
+            if rank != 0:
+                return 0
+
+        # ---- e2e through the C-ABI call with HOST buffers (H2D of K,G and D2H of C inside the timed region)
+        e2e = None
+        if rank == 0:
+            Kh = torch.from_numpy(K).pin_memory()
+            Gh = torch.from_numpy(G).pin_memory()
+            stage = torch.empty(2 * N, dtype=torch.float64, device=dev)
+            binding.solve_image_host(Kh, Gh, tol=1e-300, maxiter=3, ncheck=args.ncheck, stage=stage, workspace=s.workspace)
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            _, iters, _ = binding.solve_image_host(Kh, Gh, eps0=args.eps0, tol=1e-300, maxiter=args.e2e_iters,
+                                                   ncheck=args.ncheck, stage=stage, workspace=s.workspace)
+            torch.cuda.synchronize(dev)
+            dt = time.perf_counter() - t0
+            nsteps = sum(iters)
+            e2e = {"value": N * nsteps / dt, "unit": "voxel-updates/s",
+                   "h2d_bytes_per_step": 2 * N * 8 / nsteps, "d2h_bytes_per_step": (36 * 8 + 6 * 8 * (args.e2e_iters // args.ncheck)) / nsteps,
+                   "call": "dr_solve_image_host: H2D K,G + dr_create + 6 load cases x %d iterations + C read back" % args.e2e_iters,
+                   "seconds": dt}
+            del stage, Kh, Gh
+            # the solver's workspace was reused by the e2e call: rebuild the handle state
+            s.close()
+            s = binding.Solver(Kd, Gd, stream=stream, workspace=s.workspace, ncheck=args.ncheck, kernel=args.kernel)
+
+        tts = None
+        if args.time_to_solution and rank == 0:
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            C, log = s.solve_all(args.eps0, args.tol, 100 * n)
+            torch.cuda.synchronize(dev)
+            tts = {"seconds": time.perf_counter() - t0, "tol": args.tol,
+                   "iters": [l[1] for l in log], "status": [l[0] for l in log], "residual": [l[2] for l in log],
+                   "C": [[float("%.6f" % v) for v in row] for row in C]}
+
+    peak, peak_src = measured_peak()
+    value = world * N * args.steps / (ms * 1e-3)
+    teff = BYTES_PER_VOXEL_ITER * N * args.steps / (ms * 1e-3) / 1e9
+    kern_gbs = BYTES_PER_VOXEL_ITER * N / (kms * 1e-3) / 1e9
+    line = {
+        "metric": "pt_voxel_updates_per_s", "value": value, "unit": "voxel-updates/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s: %s" % (args.workload, WORKLOADS[args.workload]["desc"]), "grid": [n, n, n],
+                   "load_case": lc, "ncheck": args.ncheck, "kernel": "fused" if args.kernel == 0 else "split",
+                   "parallelism": "load cases sharded over %d GPU(s), no collective" % world,
+                   "l2": "inputs (%.1f GB per iteration) larger than L2; no flush needed" % (BYTES_PER_VOXEL_ITER * N / 1e9)},
+        "T_eff_GBs": teff, "T_eff_frac_of_measured_peak": teff / peak, "T_eff_frac_of_8000_nominal": teff / 8000.0,
+        "clocks": clocks,
+        "e2e": e2e,
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "hbm", "kernel": "k_pt_fused" if args.kernel == 0 else "k_stress_split+k_velocity_split",
+                     "achieved": kern_gbs, "peak": peak, "unit": "GB/s", "frac": kern_gbs / peak,
+                     "traffic": None, "peak_source": peak_src, "launch_ms": kms,
+                     "algorithmic_bytes_per_launch": BYTES_PER_VOXEL_ITER * N},
+    }
+    if tts is not None:
+        line["time_to_full_C"] = tts
+    if not args.no_cpu_baseline:
+        rate, dt, m = oracle_rate(K, G, lc, args.eps0, args.cpu_sample_n, args.cpu_iters)
+        line["cpu_baseline"] = {"value": rate, "unit": "voxel-updates/s", "cores": host_threads(), "kind": "oracle",
+                                "sample": "%d^3 crop of the same image, %d oracle PT iterations, %.1f s" % (m, args.cpu_iters, dt)}
+    print(json.dumps(line))
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

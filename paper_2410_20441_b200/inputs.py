@@ -87,7 +87,7 @@ def config4_grf(n=479, ell=12.0, soft_fraction=0.15, seed=20241021, matrix=QUART
     F = np.fft.rfftn(w)
     del w
     F *= np.exp(-(kx * kx + ky * ky + kz * kz) * (ell * ell / 8.0))
-    f = np.fft.irfftn(F, s=(n, n, n))
+    f = np.fft.irfftn(F, s=(n, n, n), axes=(0, 1, 2))
     del F
     thr = np.quantile(f, soft_fraction)
     m = f < thr
