@@ -56,7 +56,9 @@ typedef enum {
     DR_GAVG = 3,       /* shear modulus on edges: 0 harmonic mean of the 4 cells [default], 1 arithmetic (R4) */
     DR_VOID_REL = 4,   /* r>0: cells with K+4G/3 <= r*max(K+4G/3) become exact void K=G=0 [0 = off] (R9)      */
     DR_BC_MODE = 5,    /* 0 paper's mixed BCs [default]; 1 full kinematic uniform BC on all faces (R5)        */
-    DR_KERNEL = 6      /* 0 fused z-march kernel [default]; 1 split stress/velocity kernels (baseline)        */
+    DR_KERNEL = 6,     /* 0 fused z-march kernel with TMA staging [default]; 1 split stress/velocity kernels
+                          (baseline); 2 fused z-march kernel with register-prefetched LDG loads              */
+    DR_ZCHUNK = 7    /* z layers per CTA of the fused kernels; 0 = automatic [default] (tuning knob)            */
 } dr_param;
 
 /* Bytes of device workspace dr_create needs for an nx*ny*nz grid (0 if the sizes are invalid). */

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <string>
 #include <algorithm>
 
@@ -13,6 +14,7 @@
 #include "dr_kernels_aux.cuh"
 #include "dr_kernels_split.cuh"
 #include "dr_kernels_fused.cuh"
+#include "dr_kernels_tma.cuh"
 
 #define FUSED_TX 32
 #define FUSED_TY 16
@@ -51,6 +53,8 @@ struct dr_handle {
     double residual, ms;
     long long launches;
     int fused_lz;
+    CUtensorMap tm_state[2][F_COUNT];   // TMA descriptors of the padded boxes (both ping-pong buffers)
+    CUtensorMap tm_K, tm_G;
     std::string err;
 };
 
@@ -84,15 +88,20 @@ extern "C" size_t dr_workspace_bytes(int nx, int ny, int nz) {
     return (size_t)N_BIG * field_bytes(L) + SMALL_BYTES;
 }
 
-// z-chunk length of the fused kernel: make the CTA count fill whole waves of 148 SMs while keeping the
-// priming overhead (one extra step per chunk) small
+// z-chunk length of the fused kernels: make the CTA count fill whole waves of 148 SMs while keeping the priming
+// overhead (one extra step per chunk) small.  Chunks are capped at DR_LZ_MAX layers: measured on B200, CTAs of
+// neighbouring tiles drift apart on longer marches and the halo rows/columns they share stop hitting in L2
+// (479^3: 3.53 ms/iteration at 24-32 layers per chunk, 3.67 at 48, 4.37 at 64, 5.2 at 96).
+#define DR_LZ_MAX 40
 static int choose_lz(const DrLayout& L) {
     const int tiles = ((L.nx + 1 + FUSED_TX - 3) / (FUSED_TX - 2)) * ((L.ny + 1 + FUSED_TY - 3) / (FUSED_TY - 2));
     const int layers = L.nz + 1;
-    int best_lz = layers;
+    int best_lz = layers < DR_LZ_MAX ? layers : DR_LZ_MAX;
     double best = -1.0;
-    for (int c = 1; c <= 64 && c <= layers; ++c) {
+    for (int c = 1; c <= layers; ++c) {
         int lz = (layers + c - 1) / c;
+        if (lz > DR_LZ_MAX) continue;
+        if (lz < 8 && best >= 0.0) break;
         int chunks = (layers + lz - 1) / lz;
         double blocks = (double)tiles * chunks;
         double waves = std::ceil(blocks / 148.0);
@@ -100,6 +109,37 @@ static int choose_lz(const DrLayout& L) {
         if (eff > best + 1e-9) { best = eff; best_lz = lz; }
     }
     return best_lz;
+}
+
+// TMA descriptor of one padded field: 3-D fp64 tensor (PX,PY,PZ), box (FUSED_TX, FUSED_TY, 1), no swizzle,
+// out-of-range elements read as zero.  cuTensorMapEncodeTiled is fetched through the runtime (no -lcuda).
+typedef CUresult (*dr_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static bool make_tmap(dr_handle* H, dr_encode_fn enc, CUtensorMap* out, double* base) {
+    const DrLayout& L = H->L;
+    cuuint64_t dims[3] = {(cuuint64_t)L.PX, (cuuint64_t)L.PY, (cuuint64_t)L.PZ};
+    cuuint64_t strides[2] = {(cuuint64_t)L.PX * 8, (cuuint64_t)L.PX * L.PY * 8};
+    cuuint32_t box[3] = {FUSED_TX, FUSED_TY, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    const CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_NONE;   // 64/128/256 B measured: no difference
+    CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { H->err = "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")"; return false; }
+    return true;
+}
+
+static bool make_all_tmaps(dr_handle* H) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn) {
+        H->err = "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled) failed";
+        return false;
+    }
+    dr_encode_fn enc = (dr_encode_fn)fn;
+    for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) if (!make_tmap(H, enc, &H->tm_state[b][f], H->buf[b][f])) return false;
+    return make_tmap(H, enc, &H->tm_K, H->K) && make_tmap(H, enc, &H->tm_G, H->G);
 }
 
 extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K, const double* G,
@@ -160,6 +200,13 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (!cuda_ok(H, e, "cudaFuncSetAttribute")) { st = DR_ERR_CUDA; break; }
+        const int smem_t = (int)DrTmaCfg2<FUSED_TX, FUSED_TY>::SMEM2;
+        e = cudaFuncSetAttribute(k_pt_tma<0, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<0, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<1, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<1, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t);
+        if (!cuda_ok(H, e, "cudaFuncSetAttribute(k_pt_tma)")) { st = DR_ERR_CUDA; break; }
+        if (!make_all_tmaps(H)) { st = DR_ERR_CUDA; break; }
     } while (0);
     if (st != DR_OK) {
         if (H->pinned) cudaFreeHost(H->pinned);
@@ -181,7 +228,8 @@ extern "C" dr_status dr_set_param(dr_handle* H, int id, double v) {
         case DR_GAVG:      if (v != 0.0 && v != 1.0) break; H->gavg = (int)v; return DR_OK;
         case DR_VOID_REL:  if (!(v >= 0.0)) break; H->void_rel = v; return DR_OK;
         case DR_BC_MODE:   if (v != 0.0 && v != 1.0) break; H->bc_mode = (int)v; return DR_OK;
-        case DR_KERNEL:    if (v != 0.0 && v != 1.0) break; H->kernel = (int)v; return DR_OK;
+        case DR_KERNEL:    if (v != 0.0 && v != 1.0 && v != 2.0) break; H->kernel = (int)v; return DR_OK;
+        case DR_ZCHUNK:    if (!(v >= 0.0) || v > 8192.0) break; H->fused_lz = v >= 1.0 ? (int)v : choose_lz(H->L); return DR_OK;
         default: break;
     }
     return fail(H, DR_ERR_ARG, "bad parameter id or value");
@@ -251,6 +299,23 @@ static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
     const int lz = H->fused_lz;
     dim3 blk(FUSED_TX, FUSED_TY, 1);
     dim3 grd((L.nx + 1 + FUSED_TX - 3) / (FUSED_TX - 2), (L.ny + 1 + FUSED_TY - 3) / (FUSED_TY - 2), (L.nz + 1 + lz - 1) / lz);
+    if (H->kernel == 0) {
+        DrTmaps T;
+        const int c = H->cur;
+        T.m[0] = H->tm_state[c][F_VX]; T.m[1] = H->tm_state[c][F_VY]; T.m[2] = H->tm_state[c][F_VZ]; T.m[3] = H->tm_G;
+        T.m[4] = H->tm_K; T.m[5] = H->tm_state[c][F_SXX]; T.m[6] = H->tm_state[c][F_SYY]; T.m[7] = H->tm_state[c][F_SZZ];
+        T.m[8] = H->tm_state[c][F_TXY]; T.m[9] = H->tm_state[c][F_TXZ]; T.m[10] = H->tm_state[c][F_TYZ];
+        T.l2_hint = 0x1000000000000000ull;      // L2 evict_normal (evict_first measured 20 % slower, evict_last no gain)
+        const size_t smem_t = DrTmaCfg2<FUSED_TX, FUSED_TY>::SMEM2;
+        DrFields Bo = fields_of(H, c ^ 1);
+        if (H->gavg) { if (with_res) k_pt_tma<1, 1, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits);
+                       else          k_pt_tma<1, 0, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); }
+        else         { if (with_res) k_pt_tma<0, 1, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits);
+                       else          k_pt_tma<0, 0, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); }
+        CKL("k_pt_tma");
+        H->cur ^= 1;
+        return DR_OK;
+    }
     const size_t smem = DrFusedCfg<FUSED_TX, FUSED_TY>::SMEM;
     DrConstFields A = cfields_of(H, H->cur);
     DrFields B = fields_of(H, H->cur ^ 1);

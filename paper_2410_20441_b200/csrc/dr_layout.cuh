@@ -4,15 +4,17 @@
 // box of PX*PY*PZ doubles, so one linear offset q addresses the node (i,j,k) of every field:
 //     q(i,j,k) = origin + i + PX*j + PX*PY*k,   origin = OX + PX*(1 + PY)
 // Logical node ranges (staggered grid, sec. 3.3): cells [0,nx), faces/edges up to nx inclusive; the box
-// additionally holds a halo: OX = 16 doubles (one 128-byte line) to the left in x so that i = 0 is 128-byte
-// aligned when PX is a multiple of 16, one node below in y and z, and at least one node above in x, y, z.
+// additionally holds a halo: OX = 17 doubles to the left in x, one node below in y and z, and at least one
+// node above in x, y, z.  OX is odd so that the TMA boxes of the fused kernel, which start one node left of
+// an even tile origin (i0 - 1), begin at an even element = 16-byte aligned address (TMA faults otherwise);
+// PX is a multiple of 16 so that every row starts on a 128-byte line.
 // Halo content: state fields 0 (never written), moduli replicate-padded (mirror image of the nearest cell,
 // Reading R4), so kernels need no index clamping.
 #pragma once
 #include <cstddef>
 #include <cstdint>
 
-#define DR_OX 16
+#define DR_OX 17
 
 struct DrLayout {
     int nx, ny, nz;
@@ -27,7 +29,8 @@ static inline int dr_round_up(int a, int m) { return (a + m - 1) / m * m; }
 static inline DrLayout dr_make_layout(int nx, int ny, int nz) {
     DrLayout L;
     L.nx = nx; L.ny = ny; L.nz = nz;
-    L.PX = dr_round_up(DR_OX + nx + 2, 16);     // i in [-16, nx+1]
+    L.PX = dr_round_up(DR_OX + nx + 2, 16);     // i in [-17, nx+1]
+    if (L.PX % 64 == 0) L.PX += 16;              // keep the row pitch off multiples of 512 B
     L.PY = ny + 3;                               // j in [-1, ny+1]
     L.PZ = nz + 3;                               // k in [-1, nz+1]
     L.sy = L.PX;
