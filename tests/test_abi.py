@@ -35,8 +35,8 @@ def test_workspace_bytes_host_logic(libdr):
     from paper_2410_20441_b200 import binding
     assert binding.workspace_bytes(1, 8, 8) == 0 and binding.workspace_bytes(8, 8, 0) == 0
     b32 = binding.workspace_bytes(32, 32, 32)
-    # 22 padded boxes of 64 x 35 x 35 doubles (+ small scratch)
-    assert 22 * 64 * 35 * 35 * 8 <= b32 <= 22 * 64 * 35 * 35 * 8 + 22 * 256 + 65536
+    # 22 padded boxes of PX x 35 x 35 doubles (+ small scratch); PX = 17 + 34 rounded up to 64, +16 off the 512 B pitch
+    assert 22 * 80 * 35 * 35 * 8 <= b32 <= 22 * 80 * 35 * 35 * 8 + 22 * 256 + 65536
     assert binding.workspace_bytes(703, 703, 703) < 70e9          # config 5 fits one B200 (180 GB)
 
 
