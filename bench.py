@@ -175,7 +175,7 @@ def main():
     ap.add_argument("--lc", type=int, default=2)
     ap.add_argument("--eps0", type=float, default=1e-4)
     ap.add_argument("--ncheck", type=int, default=100)
-    ap.add_argument("--kernel", type=int, default=0, help="0 fused (default), 1 split baseline")
+    ap.add_argument("--kernel", type=int, default=0, help="0 fused with TMA staging (default), 1 split baseline, 2 fused with LDG prefetch")
     ap.add_argument("--cpu-sample-n", type=int, default=191)
     ap.add_argument("--cpu-iters", type=int, default=100)
     ap.add_argument("--cpu-iters-per-step", type=int, default=5)
@@ -294,14 +294,14 @@ def main():
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s: %s" % (args.workload, WORKLOADS[args.workload]["desc"]), "grid": [n, n, n],
-                   "load_case": lc, "ncheck": args.ncheck, "kernel": "fused" if args.kernel == 0 else "split",
+                   "load_case": lc, "ncheck": args.ncheck, "kernel": {0: "fused+TMA", 1: "split", 2: "fused+LDG"}[args.kernel],
                    "parallelism": "load cases sharded over %d GPU(s), no collective" % world,
                    "l2": "inputs (%.1f GB per iteration) larger than L2; no flush needed" % (BYTES_PER_VOXEL_ITER * N / 1e9)},
         "T_eff_GBs": teff, "T_eff_frac_of_measured_peak": teff / peak, "T_eff_frac_of_8000_nominal": teff / 8000.0,
         "clocks": clocks,
         "e2e": e2e,
         "gpu_launches": int(launches),
-        "roofline": {"bound": "hbm", "kernel": "k_pt_fused" if args.kernel == 0 else "k_stress_split+k_velocity_split",
+        "roofline": {"bound": "hbm", "kernel": {0: "k_pt_tma", 1: "k_stress_split+k_velocity_split", 2: "k_pt_fused"}[args.kernel],
                      "achieved": kern_gbs, "peak": peak, "unit": "GB/s", "frac": kern_gbs / peak,
                      "traffic": None, "peak_source": peak_src, "launch_ms": kms,
                      "algorithmic_bytes_per_launch": BYTES_PER_VOXEL_ITER * N},
