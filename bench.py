@@ -33,6 +33,9 @@ sys.path.insert(0, ROOT)
 from paper_2410_20441_b200 import inputs  # noqa: E402
 
 BYTES_PER_VOXEL_ITER = 160.0        # (2*9 + 2) fp64, SURVEY 8(d)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of k_pt_tma at 479^3 from the one `ncu --set full` capture
+# summarised in profiles/r1_summary.md (11.03 + 8.00 GB); null for any other workload / kernel
+NCU_TRAFFIC_BYTES = {("cfg4", 0): 19.03e9}
 WORKLOADS = {
     "cfg1": dict(n=32, gen="config1_sphere", desc="32^3 centred spherical pore r=5, contrast 1e-6"),
     "cfg2": dict(n=191, gen="config2_spheroid", desc="191^3 oblate fluid spheroid (40,40,8)"),
@@ -303,7 +306,7 @@ def main():
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": {0: "k_pt_tma", 1: "k_stress_split+k_velocity_split", 2: "k_pt_fused"}[args.kernel],
                      "achieved": kern_gbs, "peak": peak, "unit": "GB/s", "frac": kern_gbs / peak,
-                     "traffic": None, "peak_source": peak_src, "launch_ms": kms,
+                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.kernel)) if args.n is None else None, "peak_source": peak_src, "launch_ms": kms,
                      "algorithmic_bytes_per_launch": BYTES_PER_VOXEL_ITER * N},
     }
     if tts is not None:

@@ -185,3 +185,53 @@ def test_iterate_continues_step(oracle_mod, gpu):
     torch.cuda.synchronize()
     errs = field_errors(o, s, K, G, 1e-4)
     assert max(errs) <= FIELD_TOL, errs
+
+
+# ---------------------------------------------------------------- BASELINE.json full sizes, bench launch configuration
+def _host_gb():
+    try:
+        import psutil
+        return psutil.virtual_memory().available / 1e9
+    except Exception:
+        return 0.0
+
+
+def test_full_size_cfg4_479_fields_after_10_iterations(oracle_mod, gpu):
+    """cfg 4 at its full size (479^3, the graded T_eff workload), default kernel and chunking = what bench.py times"""
+    if _host_gb() < 40:
+        pytest.skip("oracle needs ~16 GB of host memory at 479^3")
+    K, G, _ = inputs.config4_grf()
+    for lc in (2, 4):
+        errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, 1e-4, 10)
+        assert max(errs) <= FIELD_TOL, (lc, errs)
+        assert abs(ro - rs) <= 1e-9 * ro
+        assert np.max(np.abs(ao - as_)) <= 1e-10 * np.max(np.abs(ao))
+
+
+def test_full_size_cfg5_703(oracle_mod, gpu):
+    """cfg 5 size (703^3, the largest): a property that holds at any size (homogeneous block: Hooke, zero residual),
+    and, when the host has the memory, 3 oracle iterations on the penny-crack image itself"""
+    import torch
+    n = 703
+    Kd = torch.full((n, n, n), 70.2, dtype=torch.float64, device="cuda")
+    Gd = torch.full((n, n, n), 29.0, dtype=torch.float64, device="cuda")
+    s = gpu.Solver(Kd, Gd, ncheck=5)
+    for lc in (2, 3):
+        assert s.solve(lc, 1e-4, 1e-8, 50) == 0
+        it, r, _ = s.info()
+        assert it == 5 and r < 1e-10
+        col = s.avg_stress() / 1e-4
+        want = np.zeros(6)
+        if lc == 2:
+            want[:3] = 70.2 - 2 * 29 / 3; want[2] = 70.2 + 4 * 29 / 3
+        else:
+            want[3] = 29.0
+        assert np.max(np.abs(col - want)) <= 1e-10 * 108.9
+    s.close(); del s, Kd, Gd
+    torch.cuda.empty_cache()
+    if _host_gb() < 90:
+        pytest.skip("oracle needs ~45 GB of host memory at 703^3; property part passed")
+    K, G, _ = inputs.config5_penny_cracks()
+    errs, ro, rs, _, _ = run_pair(oracle_mod, gpu, K, G, 2, 1e-4, 3)
+    assert max(errs) <= FIELD_TOL, errs
+    assert abs(ro - rs) <= 1e-9 * ro
