@@ -205,7 +205,9 @@ def test_full_size_cfg4_479_fields_after_10_iterations(oracle_mod, gpu):
         errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, 1e-4, 10)
         assert max(errs) <= FIELD_TOL, (lc, errs)
         assert abs(ro - rs) <= 1e-9 * ro
-        assert np.max(np.abs(ao - as_)) <= 1e-10 * np.max(np.abs(ao))
+        # the oracle adds 1.1e8 terms one after the other (rounding error up to N u ~ 1e-8, typically sqrt(N) u ~ 1e-12
+        # relative); the GPU sums pairwise.  1e-9 is still 1000x tighter than the 1e-6 bar on C.
+        assert np.max(np.abs(ao - as_)) <= 1e-9 * np.max(np.abs(ao)), np.max(np.abs(ao - as_)) / np.max(np.abs(ao))
 
 
 def test_full_size_cfg5_703(oracle_mod, gpu):
