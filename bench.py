@@ -30,7 +30,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2410_20441_b200 import inputs  # noqa: E402
+from paper_2410_20441_b200 import inputs, shard  # noqa: E402
 
 BYTES_PER_VOXEL_ITER = 160.0        # (2*9 + 2) fp64, SURVEY 8(d)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_pt_tma at 479^3 from the one `ncu --set full` capture
@@ -211,7 +211,7 @@ def main():
     N = n ** 3
     Kd = torch.from_numpy(K).to(dev)
     Gd = torch.from_numpy(G).to(dev)
-    lc = (args.lc + rank) % 6 if world > 1 else args.lc
+    lc = shard.load_case_of_rank(rank, world, args.lc)
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
         s = binding.Solver(Kd, Gd, stream=stream, ncheck=args.ncheck, kernel=args.kernel)
@@ -246,9 +246,7 @@ def main():
         kms = k0.elapsed_time(k1) / args.steps
         clocks = sampler.stop() if rank == 0 else None
         if dist is not None:
-            t = torch.tensor([ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+            ms = shard.max_over_ranks(ms, dist, dev)
             dist.barrier()
             dist.destroy_process_group()
             dist = None
@@ -289,7 +287,7 @@ def main():
                    "C": [[float("%.6f" % v) for v in row] for row in C]}
 
     peak, peak_src = measured_peak()
-    value = world * N * args.steps / (ms * 1e-3)
+    value = shard.job_throughput(N, args.steps, world, ms)
     teff = BYTES_PER_VOXEL_ITER * N * args.steps / (ms * 1e-3) / 1e9
     kern_gbs = BYTES_PER_VOXEL_ITER * N / (kms * 1e-3) / 1e9
     line = {

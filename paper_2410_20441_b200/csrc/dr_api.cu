@@ -89,24 +89,21 @@ extern "C" size_t dr_workspace_bytes(int nx, int ny, int nz) {
 }
 
 // z-chunk length of the fused kernels: make the CTA count fill whole waves of 148 SMs while keeping the priming
-// overhead (one extra step per chunk) small.  Chunks are capped at DR_LZ_MAX layers: measured on B200, CTAs of
+// overhead (one extra step per chunk) small.  Chunks are capped at DR_LZ_MAX layers (and may be as short as 1-3 layers on tiny grids, where filling the 148 SMs matters more than the priming step): measured on B200, CTAs of
 // neighbouring tiles drift apart on longer marches and the halo rows/columns they share stop hitting in L2
 // (479^3: 3.53 ms/iteration at 24-32 layers per chunk, 3.67 at 48, 4.37 at 64, 5.2 at 96).
-#define DR_LZ_MAX 40
+#define DR_LZ_MAX 36
+#define DR_LZ_FIXED 3      // per-CTA start-up (barrier init, first TMA round trip) in units of one z step
 static int choose_lz(const DrLayout& L) {
     const int tiles = ((L.nx + 1 + FUSED_TX - 3) / (FUSED_TX - 2)) * ((L.ny + 1 + FUSED_TY - 3) / (FUSED_TY - 2));
     const int layers = L.nz + 1;
     int best_lz = layers < DR_LZ_MAX ? layers : DR_LZ_MAX;
-    double best = -1.0;
-    for (int c = 1; c <= layers; ++c) {
-        int lz = (layers + c - 1) / c;
-        if (lz > DR_LZ_MAX) continue;
-        if (lz < 8 && best >= 0.0) break;
-        int chunks = (layers + lz - 1) / lz;
-        double blocks = (double)tiles * chunks;
-        double waves = std::ceil(blocks / 148.0);
-        double eff = blocks / (waves * 148.0) * (double)layers / ((double)chunks * (lz + 1));
-        if (eff > best + 1e-9) { best = eff; best_lz = lz; }
+    double best = 1e300;
+    for (int lz = 1; lz <= DR_LZ_MAX && lz <= layers; ++lz) {
+        const int chunks = (layers + lz - 1) / lz;
+        const double waves = std::ceil((double)tiles * chunks / 148.0);
+        const double cost = waves * (lz + 1 + DR_LZ_FIXED);          // steps on the critical path of one SM
+        if (cost < best - 1e-9 || (cost < best + 1e-9 && lz > best_lz)) { best = cost; best_lz = lz; }
     }
     return best_lz;
 }
