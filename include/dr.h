@@ -58,7 +58,11 @@ typedef enum {
     DR_BC_MODE = 5,    /* 0 paper's mixed BCs [default]; 1 full kinematic uniform BC on all faces (R5)        */
     DR_KERNEL = 6,     /* 0 fused z-march kernel with TMA staging [default]; 1 split stress/velocity kernels
                           (baseline); 2 fused z-march kernel with register-prefetched LDG loads              */
-    DR_ZCHUNK = 7    /* z layers per CTA of the fused kernels; 0 = automatic [default] (tuning knob)            */
+    DR_ZCHUNK = 7,     /* z layers per CTA of the fused kernels; 0 = automatic [default] (tuning knob)            */
+    DR_FORM = 8        /* 0 stress-relaxation form of the paper, Eq. 11-13 [default]; 1 displacement form: state u, w,
+                          w <- (1-theta) w + C~^2 h^2 F(u)/H_node, u <- u + w, stresses formed on the fly (same fixed
+                          point, 112 instead of 160 B per voxel-iteration; DR_KERNEL 0 or 1).  Setting DR_FORM also resets
+                          DR_CFL to the form's default (0.55 / 0.50: the explicit damping has less stability margin) */
 } dr_param;
 
 /* Bytes of device workspace dr_create needs for an nx*ny*nz grid (0 if the sizes are invalid). */

@@ -48,7 +48,7 @@ extern "C" {
 enum { DRO_OK = 0, DRO_ERR_ARG = 1, DRO_ERR_WORKSPACE = 2, DRO_ERR_CUDA = 3,
        DRO_ERR_DIVERGED = 4, DRO_ERR_STATE = 5, DRO_MAXITER = 6 };
 enum { DRO_CFL = 0, DRO_ST_FACTOR = 1, DRO_NCHECK = 2, DRO_GAVG = 3,
-       DRO_VOID_REL = 4, DRO_BC_MODE = 5 };
+       DRO_VOID_REL = 4, DRO_BC_MODE = 5, DRO_FORM = 8 };
 
 struct dro_handle {
     int nx, ny, nz;
@@ -58,8 +58,10 @@ struct dro_handle {
     /* parameters */
     double cfl, st_factor, void_rel;
     int ncheck, gavg, bc_mode;
+    int form;                        /* 0 stress-relaxation form of the paper (Eq. 11-13); 1 displacement form */
     /* state */
     std::vector<double> p, txx, tyy, tzz, txy, txz, tyz, vx, vy, vz;
+    std::vector<double> wx, wy, wz;  /* displacement form only: damped increments (pseudo-velocities) */
     /* edge shear moduli (O2), tabulated once per solve from K,G by Ctx::Gxy/Gxz/Gyz */
     std::vector<double> eGxy, eGxz, eGyz;
     /* results */
@@ -168,6 +170,7 @@ void init_fields(dro_handle* H, int lc, double eps0) {
     H->vx.assign((size_t)(nx + 1) * ny * nz, 0.0);
     H->vy.assign((size_t)nx * (ny + 1) * nz, 0.0);
     H->vz.assign((size_t)nx * ny * (nz + 1), 0.0);
+    H->wx.assign(H->vx.size(), 0.0); H->wy.assign(H->vy.size(), 0.0); H->wz.assign(H->vz.size(), 0.0);
     H->txy.assign((size_t)(nx + 1) * (ny + 1) * nz, 0.0);
     H->txz.assign((size_t)(nx + 1) * ny * (nz + 1), 0.0);
     H->tyz.assign((size_t)nx * (ny + 1) * (nz + 1), 0.0);
@@ -224,6 +227,8 @@ double pt_iteration(dro_handle* H, int lc, double eps0, bool want_res) {
     const double* K = H->K.data();
     const double* G = H->G.data();
     const int bcm = H->bc_mode;
+    const int form = H->form;
+    double *wx = H->wx.data(), *wy = H->wy.data(), *wz = H->wz.data();
     const double *eGxy = H->eGxy.data(), *eGxz = H->eGxz.data(), *eGyz = H->eGyz.data();
 
     /* ---- 1. stress update (Eq. 12-13, relaxation term implicit: reading R14) ---- */
@@ -234,10 +239,17 @@ double pt_iteration(dro_handle* H, int lc, double eps0, bool want_res) {
         double dyy = (vy[g.fy(i, j + 1, k)] - vy[g.fy(i, j, k)]) / h;
         double dzz = (vz[g.fz(i, j, k + 1)] - vz[g.fz(i, j, k)]) / h;
         double div = dxx + dyy + dzz;
+        if (form == 0) {
         p[q] = (p[q] - theta * K[q] * div) / (1.0 + theta);
         txx[q] = (txx[q] + theta * 2.0 * G[q] * (dxx - div / 3.0)) / (1.0 + theta);
         tyy[q] = (tyy[q] + theta * 2.0 * G[q] * (dyy - div / 3.0)) / (1.0 + theta);
         tzz[q] = (tzz[q] + theta * 2.0 * G[q] * (dzz - div / 3.0)) / (1.0 + theta);
+        } else {                 /* displacement form: stresses are Hooke's law of the current displacement */
+        p[q] = -K[q] * div;
+        txx[q] = 2.0 * G[q] * (dxx - div / 3.0);
+        tyy[q] = 2.0 * G[q] * (dyy - div / 3.0);
+        tzz[q] = 2.0 * G[q] * (dzz - div / 3.0);
+        }
     }
     /* shear stresses on edges; boundary edges per O6 rule T (ghost value so that the wall value is affine) */
     #pragma omp parallel for schedule(static)
@@ -253,7 +265,8 @@ double pt_iteration(dro_handle* H, int lc, double eps0, bool want_res) {
         if (i == 0)       dvy_dx = 2.0 * (vy[g.fy(0, j, k)] - A.u(1, 0.0, j * h, z)) / h;
         else if (i == nx) dvy_dx = 2.0 * (A.u(1, Lx, j * h, z) - vy[g.fy(nx - 1, j, k)]) / h;
         else              dvy_dx = (vy[g.fy(i, j, k)] - vy[g.fy(i - 1, j, k)]) / h;
-        txy[e] = (txy[e] + theta * eGxy[g.exy(i, j, k)] * (dvx_dy + dvy_dx)) / (1.0 + theta);
+        if (form == 0) txy[e] = (txy[e] + theta * eGxy[g.exy(i, j, k)] * (dvx_dy + dvy_dx)) / (1.0 + theta);
+        else           txy[e] = eGxy[g.exy(i, j, k)] * (dvx_dy + dvy_dx);
     }
     #pragma omp parallel for schedule(static)
     for (int k = 0; k <= nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i <= nx; ++i) {
@@ -268,7 +281,8 @@ double pt_iteration(dro_handle* H, int lc, double eps0, bool want_res) {
         if (i == 0)       dvz_dx = 2.0 * (vz[g.fz(0, j, k)] - A.u(2, 0.0, y, k * h)) / h;
         else if (i == nx) dvz_dx = 2.0 * (A.u(2, Lx, y, k * h) - vz[g.fz(nx - 1, j, k)]) / h;
         else              dvz_dx = (vz[g.fz(i, j, k)] - vz[g.fz(i - 1, j, k)]) / h;
-        txz[e] = (txz[e] + theta * eGxz[g.exz(i, j, k)] * (dvx_dz + dvz_dx)) / (1.0 + theta);
+        if (form == 0) txz[e] = (txz[e] + theta * eGxz[g.exz(i, j, k)] * (dvx_dz + dvz_dx)) / (1.0 + theta);
+        else           txz[e] = eGxz[g.exz(i, j, k)] * (dvx_dz + dvz_dx);
     }
     #pragma omp parallel for schedule(static)
     for (int k = 0; k <= nz; ++k) for (int j = 0; j <= ny; ++j) for (int i = 0; i < nx; ++i) {
@@ -283,7 +297,8 @@ double pt_iteration(dro_handle* H, int lc, double eps0, bool want_res) {
         if (j == 0)       dvz_dy = 2.0 * (vz[g.fz(i, 0, k)] - A.u(2, x, 0.0, k * h)) / h;
         else if (j == ny) dvz_dy = 2.0 * (A.u(2, x, Ly, k * h) - vz[g.fz(i, ny - 1, k)]) / h;
         else              dvz_dy = (vz[g.fz(i, j, k)] - vz[g.fz(i, j - 1, k)]) / h;
-        tyz[e] = (tyz[e] + theta * eGyz[g.eyz(i, j, k)] * (dvy_dz + dvz_dy)) / (1.0 + theta);
+        if (form == 0) tyz[e] = (tyz[e] + theta * eGyz[g.eyz(i, j, k)] * (dvy_dz + dvz_dy)) / (1.0 + theta);
+        else           tyz[e] = eGyz[g.eyz(i, j, k)] * (dvy_dz + dvz_dy);
     }
 
     /* ---- 2. velocity update with the NEW stresses (Eq. 11); wall nodes untouched (O6 rule N).
@@ -301,7 +316,8 @@ double pt_iteration(dro_handle* H, int lc, double eps0, bool want_res) {
                                       std::max(eGxz[g.exz(i, j, k)], eGxz[g.exz(i, j, k + 1)])));
         if (Hn > 0.0) {
             if (want_res) { double r = std::fabs(F) * h / (Hn * ae); if (!(r <= res)) res = r; }
-            vx[g.fx(i, j, k)] += c2 / (theta * Hn) * F;
+            if (form == 0) vx[g.fx(i, j, k)] += c2 / (theta * Hn) * F;
+            else { size_t n = g.fx(i, j, k); wx[n] = (1.0 - theta) * wx[n] + c2 / Hn * F; vx[n] += wx[n]; }
         }
     }
     #pragma omp parallel for schedule(static) reduction(max : res)
@@ -315,7 +331,8 @@ double pt_iteration(dro_handle* H, int lc, double eps0, bool want_res) {
                                       std::max(eGyz[g.eyz(i, j, k)], eGyz[g.eyz(i, j, k + 1)])));
         if (Hn > 0.0) {
             if (want_res) { double r = std::fabs(F) * h / (Hn * ae); if (!(r <= res)) res = r; }
-            vy[g.fy(i, j, k)] += c2 / (theta * Hn) * F;
+            if (form == 0) vy[g.fy(i, j, k)] += c2 / (theta * Hn) * F;
+            else { size_t n = g.fy(i, j, k); wy[n] = (1.0 - theta) * wy[n] + c2 / Hn * F; vy[n] += wy[n]; }
         }
     }
     #pragma omp parallel for schedule(static) reduction(max : res)
@@ -329,7 +346,8 @@ double pt_iteration(dro_handle* H, int lc, double eps0, bool want_res) {
                                       std::max(eGyz[g.eyz(i, j, k)], eGyz[g.eyz(i, j + 1, k)])));
         if (Hn > 0.0) {
             if (want_res) { double r = std::fabs(F) * h / (Hn * ae); if (!(r <= res)) res = r; }
-            vz[g.fz(i, j, k)] += c2 / (theta * Hn) * F;
+            if (form == 0) vz[g.fz(i, j, k)] += c2 / (theta * Hn) * F;
+            else { size_t n = g.fz(i, j, k); wz[n] = (1.0 - theta) * wz[n] + c2 / Hn * F; vz[n] += wz[n]; }
         }
     }
     return res;
@@ -384,7 +402,7 @@ int dro_create(int nx, int ny, int nz, double h, const double* K, const double* 
     dro_handle* H = new dro_handle();
     H->nx = nx; H->ny = ny; H->nz = nz; H->h = h;
     H->K0.assign(K, K + N); H->G0.assign(G, G + N);
-    H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0;
+    H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->form = 0;
     for (int a = 0; a < 6; ++a) { H->have[a] = false; for (int b = 0; b < 6; ++b) H->Ccol[a][b] = 0.0; }
     H->have_avg = false; H->iters = 0; H->residual = 0.0; H->ms = 0.0;
     *out = H;
@@ -400,6 +418,9 @@ int dro_set_param(dro_handle* H, int id, double value) {
         case DRO_GAVG:      if (value != 0.0 && value != 1.0) break; H->gavg = (int)value; return DRO_OK;
         case DRO_VOID_REL:  if (!(value >= 0.0)) break; H->void_rel = value; return DRO_OK;
         case DRO_BC_MODE:   if (value != 0.0 && value != 1.0) break; H->bc_mode = (int)value; return DRO_OK;
+        /* the explicit damping of the displacement form has a smaller stability margin (diverges at C~ = 0.55 on
+           small grids, converges at 0.52): choosing a form also resets C~ to that form's default */
+        case DRO_FORM:      if (value != 0.0 && value != 1.0) break; H->form = (int)value; H->cfl = H->form ? 0.50 : 0.55; return DRO_OK;
         default: break;
     }
     H->err = "bad parameter id or value";

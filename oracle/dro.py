@@ -18,6 +18,7 @@ _LIB = os.path.join(_HERE, "libdro.so")
 
 OK, ERR_ARG, ERR_WORKSPACE, ERR_CUDA, ERR_DIVERGED, ERR_STATE, MAXITER = range(7)
 CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE = range(6)
+FORM = 8
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
 
 
@@ -88,7 +89,7 @@ class Oracle:
         return st
 
     def set_param(self, name, value):
-        ids = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE)
+        ids = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, form=FORM)
         self._check(lib().dro_set_param(self._h, ids[name], float(value)))
 
     def solve(self, lc, eps0=1e-4, tol=1e-8, maxiter=100000):

@@ -13,8 +13,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdr.so")
 
 OK, ERR_ARG, ERR_WORKSPACE, ERR_CUDA, ERR_DIVERGED, ERR_STATE, MAXITER = range(7)
-CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK = range(8)
-PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK)
+CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK, FORM = range(9)
+PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK, form=FORM)
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
 EXPORTS = ("dr_workspace_bytes", "dr_create", "dr_set_param", "dr_solve", "dr_step", "dr_iterate",
            "dr_effective_C", "dr_avg_stress", "dr_info", "dr_get_field", "dr_solve_image_host",

@@ -36,11 +36,12 @@ struct dr_handle {
     cudaEvent_t e0, e1;
     // parameters
     double cfl, st_factor, void_rel;
-    int ncheck, gavg, bc_mode, kernel;
+    int ncheck, gavg, bc_mode, kernel, form;
     double void_applied;        // void_rel currently baked into K,G
     double hmax;
     // state
     int cur;                    // ping-pong buffer that holds the current fields
+    bool stress_stale;          // DR_FORM 1 with the fused kernel: stresses not yet formed from the displacement
     bool have_fields;
     int cur_lc;
     double cur_eps0;
@@ -162,7 +163,7 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
     H->hmax_bits = (unsigned long long*)p; p += 256;
     H->flags = (unsigned int*)p; p += 256;
     H->pinned = nullptr; H->e0 = H->e1 = nullptr;
-    H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->kernel = 0;
+    H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->kernel = 0; H->form = 0;
     H->void_applied = 0.0; H->hmax = 0.0;
     H->cur = 0; H->have_fields = false; H->cur_lc = -1; H->cur_eps0 = 0.0;
     for (int a = 0; a < 6; ++a) { H->have[a] = false; H->avg[a] = 0; for (int b = 0; b < 6; ++b) H->Ccol[a][b] = 0.0; }
@@ -198,10 +199,10 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (!cuda_ok(H, e, "cudaFuncSetAttribute")) { st = DR_ERR_CUDA; break; }
         const int smem_t = (int)DrTmaCfg2<FUSED_TX, FUSED_TY>::SMEM2;
-        e = cudaFuncSetAttribute(k_pt_tma<0, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<0, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<1, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<1, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t);
+#define DR_SET_TMA_ATTR(G_, R_, F_) if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<G_, R_, F_, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t)
+        DR_SET_TMA_ATTR(0, 0, 0); DR_SET_TMA_ATTR(0, 1, 0); DR_SET_TMA_ATTR(1, 0, 0); DR_SET_TMA_ATTR(1, 1, 0);
+        DR_SET_TMA_ATTR(0, 0, 1); DR_SET_TMA_ATTR(0, 1, 1); DR_SET_TMA_ATTR(1, 0, 1); DR_SET_TMA_ATTR(1, 1, 1);
+#undef DR_SET_TMA_ATTR
         if (!cuda_ok(H, e, "cudaFuncSetAttribute(k_pt_tma)")) { st = DR_ERR_CUDA; break; }
         if (!make_all_tmaps(H)) { st = DR_ERR_CUDA; break; }
     } while (0);
@@ -226,6 +227,9 @@ extern "C" dr_status dr_set_param(dr_handle* H, int id, double v) {
         case DR_VOID_REL:  if (!(v >= 0.0)) break; H->void_rel = v; return DR_OK;
         case DR_BC_MODE:   if (v != 0.0 && v != 1.0) break; H->bc_mode = (int)v; return DR_OK;
         case DR_KERNEL:    if (v != 0.0 && v != 1.0 && v != 2.0) break; H->kernel = (int)v; return DR_OK;
+        // choosing a form also resets C~ to that form's default (the explicit damping of the displacement form
+        // diverges at 0.55 on small grids)
+        case DR_FORM:      if (v != 0.0 && v != 1.0) break; H->form = (int)v; H->cfl = H->form ? 0.50 : 0.55; H->have_fields = false; return DR_OK;
         case DR_ZCHUNK:    if (!(v >= 0.0) || v > 8192.0) break; H->fused_lz = v >= 1.0 ? (int)v : choose_lz(H->L); return DR_OK;
         default: break;
     }
@@ -269,10 +273,11 @@ static dr_status prepare(dr_handle* H, int lc, double eps0) {
     }
     DrPT P = make_pt(H, lc, eps0);
     dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
-    if (H->gavg) k_bc_init<1><<<grd, blk, 0, H->st>>>(H->L, P, fields_of(H, 0), H->K, H->G);
-    else         k_bc_init<0><<<grd, blk, 0, H->st>>>(H->L, P, fields_of(H, 0), H->K, H->G);
+    if (H->form == 1 && H->kernel == 2) return fail(H, DR_ERR_ARG, "DR_FORM = 1 is implemented by DR_KERNEL 0 and 1 only");
+    if (H->gavg) k_bc_init<1><<<grd, blk, 0, H->st>>>(H->L, P, fields_of(H, 0), fields_of(H, 1), H->form, H->K, H->G);
+    else         k_bc_init<0><<<grd, blk, 0, H->st>>>(H->L, P, fields_of(H, 0), fields_of(H, 1), H->form, H->K, H->G);
     CKL("k_bc_init");
-    H->cur = 0; H->have_fields = true; H->cur_lc = lc; H->cur_eps0 = eps0;
+    H->cur = 0; H->have_fields = true; H->cur_lc = lc; H->cur_eps0 = eps0; H->stress_stale = false;
     return DR_OK;
 }
 
@@ -281,15 +286,18 @@ static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
     const DrLayout& L = H->L;
     if (H->kernel == 1) {
         dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
-        DrFields F = fields_of(H, H->cur);
-        if (H->gavg) k_stress_split<1><<<grd, blk, 0, H->st>>>(H->L, P, F, H->K, H->G);
-        else         k_stress_split<0><<<grd, blk, 0, H->st>>>(H->L, P, F, H->K, H->G);
-        CKL("k_stress_split");
+        // FORM 0: in place in buffer cur.  FORM 1: u, w in buffer cur, stresses of this iteration in buffer cur^1.
+        DrFields U = fields_of(H, H->cur);
+        DrFields S = fields_of(H, H->form ? H->cur ^ 1 : H->cur);
+        DrConstFields Uc = cfields_of(H, H->cur), Sc = cfields_of(H, H->form ? H->cur ^ 1 : H->cur);
         dim3 grv((L.nx + 63) / 64, (L.ny + 3) / 4, L.nz);
-        if (H->gavg) { if (with_res) k_velocity_split<1, 1><<<grv, blk, 0, H->st>>>(H->L, P, F, H->K, H->G, H->res_bits);
-                       else          k_velocity_split<1, 0><<<grv, blk, 0, H->st>>>(H->L, P, F, H->K, H->G, H->res_bits); }
-        else         { if (with_res) k_velocity_split<0, 1><<<grv, blk, 0, H->st>>>(H->L, P, F, H->K, H->G, H->res_bits);
-                       else          k_velocity_split<0, 0><<<grv, blk, 0, H->st>>>(H->L, P, F, H->K, H->G, H->res_bits); }
+#define DR_SPLIT(G_, F_) do { \
+            k_stress_split<G_, F_><<<grd, blk, 0, H->st>>>(H->L, P, Uc, S, H->K, H->G); CKL("k_stress_split"); \
+            if (with_res) k_velocity_split<G_, 1, F_><<<grv, blk, 0, H->st>>>(H->L, P, U, Sc, H->K, H->G, H->res_bits); \
+            else          k_velocity_split<G_, 0, F_><<<grv, blk, 0, H->st>>>(H->L, P, U, Sc, H->K, H->G, H->res_bits); } while (0)
+        if (H->gavg) { if (H->form) DR_SPLIT(1, 1); else DR_SPLIT(1, 0); }
+        else         { if (H->form) DR_SPLIT(0, 1); else DR_SPLIT(0, 0); }
+#undef DR_SPLIT
         CKL("k_velocity_split");
         return DR_OK;
     }
@@ -305,12 +313,16 @@ static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
         T.l2_hint = 0x1000000000000000ull;      // L2 evict_normal (evict_first measured 20 % slower, evict_last no gain)
         const size_t smem_t = DrTmaCfg2<FUSED_TX, FUSED_TY>::SMEM2;
         DrFields Bo = fields_of(H, c ^ 1);
-        if (H->gavg) { if (with_res) k_pt_tma<1, 1, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits);
-                       else          k_pt_tma<1, 0, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); }
-        else         { if (with_res) k_pt_tma<0, 1, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits);
-                       else          k_pt_tma<0, 0, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); }
+#define DR_TMA(G_, R_, F_) k_pt_tma<G_, R_, F_, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits)
+        const int sel = (H->gavg ? 4 : 0) | (with_res ? 2 : 0) | (H->form ? 1 : 0);
+        switch (sel) {
+            case 0: DR_TMA(0, 0, 0); break; case 1: DR_TMA(0, 0, 1); break; case 2: DR_TMA(0, 1, 0); break; case 3: DR_TMA(0, 1, 1); break;
+            case 4: DR_TMA(1, 0, 0); break; case 5: DR_TMA(1, 0, 1); break; case 6: DR_TMA(1, 1, 0); break; default: DR_TMA(1, 1, 1); break;
+        }
+#undef DR_TMA
         CKL("k_pt_tma");
         H->cur ^= 1;
+        if (H->form) H->stress_stale = true;
         return DR_OK;
     }
     const size_t smem = DrFusedCfg<FUSED_TX, FUSED_TY>::SMEM;
@@ -325,6 +337,23 @@ static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
     return DR_OK;
 }
 
+// buffer whose stress slots hold the stresses: in the displacement form the sigma_aa slots of the state buffer carry
+// w, and the stresses (Hooke's law of the displacement BEFORE the last update, like the oracle's) sit in the other one
+static int stress_buf(const dr_handle* H) { return H->form ? H->cur ^ 1 : H->cur; }
+
+static dr_status ensure_stresses(dr_handle* H) {
+    if (!H->form || !H->stress_stale) return DR_OK;
+    const DrLayout& L = H->L;
+    const DrPT P = make_pt(H, H->cur_lc, H->cur_eps0);
+    const int b = H->cur ^ 1;                       // holds u before the last update; its w is dead
+    dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
+    if (H->gavg) k_stress_split<1, 1><<<grd, blk, 0, H->st>>>(H->L, P, cfields_of(H, b), fields_of(H, b), H->K, H->G);
+    else         k_stress_split<0, 1><<<grd, blk, 0, H->st>>>(H->L, P, cfields_of(H, b), fields_of(H, b), H->K, H->G);
+    CKL("k_stress_split(finalize)");
+    H->stress_stale = false;
+    return DR_OK;
+}
+
 static dr_status read_residual(dr_handle* H, double* r) {
     CK(cudaMemcpyAsync(H->pinned, H->res_bits, 8, cudaMemcpyDeviceToHost, H->st));
     CK(cudaStreamSynchronize(H->st));
@@ -334,7 +363,8 @@ static dr_status read_residual(dr_handle* H, double* r) {
 
 static dr_status averages(dr_handle* H, int lc, double eps0) {
     const DrLayout& L = H->L;
-    k_avg_partial<<<DR_AVG_BLOCKS, DR_AVG_THREADS, 0, H->st>>>(H->L, cfields_of(H, H->cur), H->partial);
+    { dr_status es = ensure_stresses(H); if (es != DR_OK) return es; }
+    k_avg_partial<<<DR_AVG_BLOCKS, DR_AVG_THREADS, 0, H->st>>>(H->L, cfields_of(H, stress_buf(H)), H->partial);
     CKL("k_avg_partial");
     k_avg_final<<<1, 256, 0, H->st>>>(H->partial, DR_AVG_BLOCKS, 1.0 / ((double)L.nx * L.ny * L.nz), H->avg_dev);
     CKL("k_avg_final");
@@ -460,7 +490,9 @@ extern "C" dr_status dr_get_field(dr_handle* H, int field, double* dst, size_t n
     }
     if (n != (size_t)ex * ey * ez) return fail(H, DR_ERR_ARG, "bad field size");
     dim3 blk(64, 4, 1), grd((ex + 63) / 64, (ey + 3) / 4, ez);
-    k_export<<<grd, blk, 0, H->st>>>(H->L, H->buf[H->cur][field], dst, ex, ey, ez);
+    { dr_status es = ensure_stresses(H); if (es != DR_OK) return es; }
+    const int src = field <= F_VZ ? H->cur : stress_buf(H);
+    k_export<<<grd, blk, 0, H->st>>>(H->L, H->buf[src][field], dst, ex, ey, ez);
     CKL("k_export");
     CK(cudaStreamSynchronize(H->st));
     return DR_OK;

@@ -57,8 +57,11 @@ __global__ void k_void_clamp(DrLayout L, const double* __restrict__ K0, const do
 // a4: initial fields and boundary values (Reading R8): every velocity node := affine u0 at its
 // own position, stresses := Hooke's law of the uniform strain (boundary shear zero where the face is free-slip,
 // App. A.1).  One thread per node of the (nx+1)(ny+1)(nz+1) box.
+// FORM 1 (displacement form): F is the state buffer (u, and w = 0 in its sigma_aa slots, zeros in
+// its shear slots) and F2 the buffer that receives u and the Hooke stresses; FORM 0: F receives everything, F2 unused.
 template <int GAVG>
-__global__ void k_bc_init(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, const double* __restrict__ Gp) {
+__global__ void k_bc_init(DrLayout L, DrPT P, DrFields F, DrFields F2, int form,
+                          const double* __restrict__ Kp, const double* __restrict__ Gp) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     int j = blockIdx.y * blockDim.y + threadIdx.y;
     int k = blockIdx.z;
@@ -71,9 +74,16 @@ __global__ void k_bc_init(DrLayout L, DrPT P, DrFields F, const double* __restri
     const double gyz = P.D[5] + P.D[7], gxz = P.D[2] + P.D[6], gxy = P.D[1] + P.D[3];
     const double trE = Exx + Eyy + Ezz;
     const bool ci = i < nx, cj = j < ny, ck = k < nz;
-    F.f[F_VX][q] = (cj && ck) ? dr_u0(P, 0, i * h, (j + 0.5) * h, (k + 0.5) * h) : 0.0;
-    F.f[F_VY][q] = (ci && ck) ? dr_u0(P, 1, (i + 0.5) * h, j * h, (k + 0.5) * h) : 0.0;
-    F.f[F_VZ][q] = (ci && cj) ? dr_u0(P, 2, (i + 0.5) * h, (j + 0.5) * h, k * h) : 0.0;
+    const double ux = (cj && ck) ? dr_u0(P, 0, i * h, (j + 0.5) * h, (k + 0.5) * h) : 0.0;
+    const double uy = (ci && ck) ? dr_u0(P, 1, (i + 0.5) * h, j * h, (k + 0.5) * h) : 0.0;
+    const double uz = (ci && cj) ? dr_u0(P, 2, (i + 0.5) * h, (j + 0.5) * h, k * h) : 0.0;
+    F.f[F_VX][q] = ux; F.f[F_VY][q] = uy; F.f[F_VZ][q] = uz;
+    if (form == 1) {
+        F.f[F_SXX][q] = 0.0; F.f[F_SYY][q] = 0.0; F.f[F_SZZ][q] = 0.0;
+        F.f[F_TXY][q] = 0.0; F.f[F_TXZ][q] = 0.0; F.f[F_TYZ][q] = 0.0;
+        F2.f[F_VX][q] = ux; F2.f[F_VY][q] = uy; F2.f[F_VZ][q] = uz;
+    }
+    DrFields& S = (form == 1) ? F2 : F;
     double sxx = 0, syy = 0, szz = 0;
     if (ci && cj && ck) {
         double Kc = Kp[q], Gc = Gp[q];
@@ -82,7 +92,7 @@ __global__ void k_bc_init(DrLayout L, DrPT P, DrFields F, const double* __restri
         syy = -pr + 2.0 * Gc * (Eyy - trE / 3.0);
         szz = -pr + 2.0 * Gc * (Ezz - trE / 3.0);
     }
-    F.f[F_SXX][q] = sxx; F.f[F_SYY][q] = syy; F.f[F_SZZ][q] = szz;
+    S.f[F_SXX][q] = sxx; S.f[F_SYY][q] = syy; S.f[F_SZZ][q] = szz;
     double txy = 0, txz = 0, tyz = 0;
     const bool bi = (i == 0 || i == nx), bj = (j == 0 || j == ny), bk = (k == 0 || k == nz);
     if (ck && (!(bi || bj) || P.ghost_xy))
@@ -91,7 +101,7 @@ __global__ void k_bc_init(DrLayout L, DrPT P, DrFields F, const double* __restri
         txz = dr_edge_mean<GAVG>(Gp[q - 1 - sz], Gp[q - sz], Gp[q - 1], Gp[q]) * gxz;
     if (ci && (!(bj || bk) || P.ghost_yz))
         tyz = dr_edge_mean<GAVG>(Gp[q - sy - sz], Gp[q - sz], Gp[q - sy], Gp[q]) * gyz;
-    F.f[F_TXY][q] = txy; F.f[F_TXZ][q] = txz; F.f[F_TYZ][q] = tyz;
+    S.f[F_TXY][q] = txy; S.f[F_TXZ][q] = txz; S.f[F_TYZ][q] = tyz;
 }
 
 // ------------------------------------------------------------------------------------------------------

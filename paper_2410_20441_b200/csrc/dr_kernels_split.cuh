@@ -14,9 +14,11 @@ __device__ __forceinline__ double dr_dshear(double v_hi, double v_lo, int e, int
 }
 
 // Eq. 12-13 with the relaxation term implicit: s <- (s + theta * Hooke(grad v)) / (1 + theta)
-template <int GAVG>
+// FORM 1 (displacement form): the stresses are Hooke's law of the displacement itself (no relaxation).
+// V = buffer whose velocity/displacement fields are read, F = buffer whose stress fields are updated.
+template <int GAVG, int FORM>
 __global__ void __launch_bounds__(256)
-k_stress_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, const double* __restrict__ Gp) {
+k_stress_split(DrLayout L, DrPT P, DrConstFields V, DrFields F, const double* __restrict__ Kp, const double* __restrict__ Gp) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     int j = blockIdx.y * blockDim.y + threadIdx.y;
     int k = blockIdx.z;
@@ -24,9 +26,9 @@ k_stress_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, co
     if (i > nx || j > ny) return;
     const long long sy = L.sy, sz = L.sz;
     const long long q = L.origin + i + sy * j + sz * k;
-    const double* __restrict__ vx = F.f[F_VX];
-    const double* __restrict__ vy = F.f[F_VY];
-    const double* __restrict__ vz = F.f[F_VZ];
+    const double* vx = V.f[F_VX];
+    const double* vy = V.f[F_VY];
+    const double* vz = V.f[F_VZ];
     const double h = P.h, ih = P.inv_h, th = P.theta, ri = P.rinv;
     const bool ci = i < nx, cj = j < ny, ck = k < nz;
     if (ci && cj && ck) {
@@ -34,9 +36,15 @@ k_stress_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, co
         double div = dxx + dyy + dzz;
         double Kc = Kp[q], Gc = Gp[q];
         double lam_div = (Kc - 2.0 * Gc / 3.0) * div;
-        F.f[F_SXX][q] = (F.f[F_SXX][q] + th * (lam_div + 2.0 * Gc * dxx)) * ri;
-        F.f[F_SYY][q] = (F.f[F_SYY][q] + th * (lam_div + 2.0 * Gc * dyy)) * ri;
-        F.f[F_SZZ][q] = (F.f[F_SZZ][q] + th * (lam_div + 2.0 * Gc * dzz)) * ri;
+        if (FORM) {
+            F.f[F_SXX][q] = lam_div + 2.0 * Gc * dxx;
+            F.f[F_SYY][q] = lam_div + 2.0 * Gc * dyy;
+            F.f[F_SZZ][q] = lam_div + 2.0 * Gc * dzz;
+        } else {
+            F.f[F_SXX][q] = (F.f[F_SXX][q] + th * (lam_div + 2.0 * Gc * dxx)) * ri;
+            F.f[F_SYY][q] = (F.f[F_SYY][q] + th * (lam_div + 2.0 * Gc * dyy)) * ri;
+            F.f[F_SZZ][q] = (F.f[F_SZZ][q] + th * (lam_div + 2.0 * Gc * dzz)) * ri;
+        }
     }
     const bool bi = (i == 0 || i == nx), bj = (j == 0 || j == ny), bk = (k == 0 || k == nz);
     if (ck) {                                   // tau_xy at (i h, j h, (k+.5) h)
@@ -46,7 +54,7 @@ k_stress_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, co
             double a = dr_dshear(vx[q], vx[q - sy], j, ny, dr_u0(P, 0, i * h, j == 0 ? 0.0 : P.Ly, z));
             double b = dr_dshear(vy[q], vy[q - 1], i, nx, dr_u0(P, 1, i == 0 ? 0.0 : P.Lx, j * h, z));
             double Ge = dr_edge_mean<GAVG>(Gp[q - 1 - sy], Gp[q - sy], Gp[q - 1], Gp[q]);
-            t = (F.f[F_TXY][q] + th * Ge * ((a + b) * ih)) * ri;
+            t = FORM ? Ge * ((a + b) * ih) : (F.f[F_TXY][q] + th * Ge * ((a + b) * ih)) * ri;
         }
         F.f[F_TXY][q] = t;
     }
@@ -57,7 +65,7 @@ k_stress_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, co
             double a = dr_dshear(vx[q], vx[q - sz], k, nz, dr_u0(P, 0, i * h, y, k == 0 ? 0.0 : P.Lz));
             double b = dr_dshear(vz[q], vz[q - 1], i, nx, dr_u0(P, 2, i == 0 ? 0.0 : P.Lx, y, k * h));
             double Ge = dr_edge_mean<GAVG>(Gp[q - 1 - sz], Gp[q - sz], Gp[q - 1], Gp[q]);
-            t = (F.f[F_TXZ][q] + th * Ge * ((a + b) * ih)) * ri;
+            t = FORM ? Ge * ((a + b) * ih) : (F.f[F_TXZ][q] + th * Ge * ((a + b) * ih)) * ri;
         }
         F.f[F_TXZ][q] = t;
     }
@@ -68,7 +76,7 @@ k_stress_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, co
             double a = dr_dshear(vy[q], vy[q - sz], k, nz, dr_u0(P, 1, x, j * h, k == 0 ? 0.0 : P.Lz));
             double b = dr_dshear(vz[q], vz[q - sy], j, ny, dr_u0(P, 2, x, j == 0 ? 0.0 : P.Ly, k * h));
             double Ge = dr_edge_mean<GAVG>(Gp[q - sy - sz], Gp[q - sz], Gp[q - sy], Gp[q]);
-            t = (F.f[F_TYZ][q] + th * Ge * ((a + b) * ih)) * ri;
+            t = FORM ? Ge * ((a + b) * ih) : (F.f[F_TYZ][q] + th * Ge * ((a + b) * ih)) * ri;
         }
         F.f[F_TYZ][q] = t;
     }
@@ -78,9 +86,11 @@ k_stress_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, co
 // H_node = stiffest of the six springs in the node's stencil (Reading R3); nodes with H_node = 0 are skipped.
 // RES: also the residual max-norm res = max |F| h / (H_node |eps0|), warp-shuffle + block
 // reduction, one atomicMax per block on the bit pattern.
-template <int GAVG, int RES>
+// FORM 1: w <- (1-theta) w + C~^2 h^2 F / H_node, u <- u + w; w lives in the sigma_aa slots of the state buffer U,
+// the stresses are read from S.  FORM 0: U and S are the same buffer.
+template <int GAVG, int RES, int FORM>
 __global__ void __launch_bounds__(256)
-k_velocity_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, const double* __restrict__ Gp,
+k_velocity_split(DrLayout L, DrPT P, DrFields U, DrConstFields S, const double* __restrict__ Kp, const double* __restrict__ Gp,
                  unsigned long long* res_bits) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -92,12 +102,12 @@ k_velocity_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, 
     double rmax = 0.0;
     bool rnan = false;
     if (i < nx && j < ny && k < nz) {
-        const double* __restrict__ sxx = F.f[F_SXX];
-        const double* __restrict__ syy = F.f[F_SYY];
-        const double* __restrict__ szz = F.f[F_SZZ];
-        const double* __restrict__ txy = F.f[F_TXY];
-        const double* __restrict__ txz = F.f[F_TXZ];
-        const double* __restrict__ tyz = F.f[F_TYZ];
+        const double* sxx = S.f[F_SXX];
+        const double* syy = S.f[F_SYY];
+        const double* szz = S.f[F_SZZ];
+        const double* txy = S.f[F_TXY];
+        const double* txz = S.f[F_TXZ];
+        const double* tyz = S.f[F_TYZ];
         auto Hc = [&](long long s) { return Kp[s] + 4.0 * Gp[s] / 3.0; };
         auto Gxy = [&](long long s) { return dr_edge_mean<GAVG>(Gp[s - 1 - sy], Gp[s - sy], Gp[s - 1], Gp[s]); };
         auto Gxz = [&](long long s) { return dr_edge_mean<GAVG>(Gp[s - 1 - sz], Gp[s - sz], Gp[s - 1], Gp[s]); };
@@ -108,7 +118,8 @@ k_velocity_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, 
             double Hn = fmax(fmax(Hc(q - 1), hq), fmax(fmax(gxy, Gxy(q + sy)), fmax(gxz, Gxz(q + sz))));
             if (Hn > 0.0) {
                 if (RES) { double r = fabs(Fx) / Hn; rnan |= !(r == r); rmax = fmax(rmax, r); }
-                F.f[F_VX][q] += P.c2t / Hn * Fx;
+                if (FORM) { double w = (1.0 - P.theta) * U.f[F_SXX][q] + P.c2t * P.theta / Hn * Fx; U.f[F_SXX][q] = w; U.f[F_VX][q] += w; }
+                else U.f[F_VX][q] += P.c2t / Hn * Fx;
             }
         }
         if (j >= 1) {
@@ -116,7 +127,8 @@ k_velocity_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, 
             double Hn = fmax(fmax(Hc(q - sy), hq), fmax(fmax(gxy, Gxy(q + 1)), fmax(gyz, Gyz(q + sz))));
             if (Hn > 0.0) {
                 if (RES) { double r = fabs(Fy) / Hn; rnan |= !(r == r); rmax = fmax(rmax, r); }
-                F.f[F_VY][q] += P.c2t / Hn * Fy;
+                if (FORM) { double w = (1.0 - P.theta) * U.f[F_SYY][q] + P.c2t * P.theta / Hn * Fy; U.f[F_SYY][q] = w; U.f[F_VY][q] += w; }
+                else U.f[F_VY][q] += P.c2t / Hn * Fy;
             }
         }
         if (k >= 1) {
@@ -124,7 +136,8 @@ k_velocity_split(DrLayout L, DrPT P, DrFields F, const double* __restrict__ Kp, 
             double Hn = fmax(fmax(Hc(q - sz), hq), fmax(fmax(gxz, Gxz(q + 1)), fmax(gyz, Gyz(q + sy))));
             if (Hn > 0.0) {
                 if (RES) { double r = fabs(Fz) / Hn; rnan |= !(r == r); rmax = fmax(rmax, r); }
-                F.f[F_VZ][q] += P.c2t / Hn * Fz;
+                if (FORM) { double w = (1.0 - P.theta) * U.f[F_SZZ][q] + P.c2t * P.theta / Hn * Fz; U.f[F_SZZ][q] = w; U.f[F_VZ][q] += w; }
+                else U.f[F_VZ][q] += P.c2t / Hn * Fz;
             }
         }
     }

@@ -63,6 +63,31 @@ __device__ __forceinline__ void dr_tma_load_3d(void* dst, const CUtensorMap* map
         ::"r"(dr_smem_u32(dst)), "l"((unsigned long long)map), "r"(dr_smem_u32(bar)), "r"(x), "r"(y), "r"(z), "l"(hint) : "memory");
 }
 
+// one batch: ring-A fields of layer m (z = m+1 in the padded box) and, if with_b, the ring-B set m:
+//   FORM 0: K, sigma_xx, sigma_yy, sigma_zz, tau_xy of layer m-1 and tau_xz, tau_yz of face m
+//   FORM 1: K, w_x, w_y, w_z of layer m-1 (w lives in the sigma_aa slots of the state buffer)
+template <int FORM, int TX, int TY>
+__device__ __forceinline__ void dr_tma_issue_batch(const DrTmaps& T, unsigned long long* bar, double* da, double* db,
+                                                   int x0, int y0, int m, bool with_b) {
+    constexpr int PL = TX * TY;
+    constexpr unsigned BA = DR_TMA_NA * PL * sizeof(double);
+    constexpr unsigned BB = (FORM ? 4 : DR_TMA_NB) * PL * sizeof(double);
+    dr_mbar_expect_tx(bar, with_b ? BA + BB : BA);
+#pragma unroll
+    for (int f = 0; f < DR_TMA_NA; ++f) dr_tma_load_3d(da + f * PL, &T.m[f], bar, x0, y0, m + 1, T.l2_hint);
+    if (with_b) {
+        if (FORM) {
+#pragma unroll
+            for (int f = 0; f < 4; ++f) dr_tma_load_3d(db + f * PL, &T.m[DR_TMA_NA + f], bar, x0, y0, m, T.l2_hint);
+        } else {
+#pragma unroll
+            for (int f = 0; f < 5; ++f) dr_tma_load_3d(db + f * PL, &T.m[DR_TMA_NA + f], bar, x0, y0, m, T.l2_hint);
+            dr_tma_load_3d(db + 5 * PL, &T.m[DR_TMA_NA + 5], bar, x0, y0, m + 1, T.l2_hint);
+            dr_tma_load_3d(db + 6 * PL, &T.m[DR_TMA_NA + 6], bar, x0, y0, m + 1, T.l2_hint);
+        }
+    }
+}
+
 // new values a thread carries from one step to the next (registers): its own tau / edge moduli on the face
 // between the layers, sigma_zz and H of the layer below, and the +x / +y neighbours' face values
 struct DrCarry { double txz, tyz, gxz, gyz, szz, hc, txz_r, tyz_u, gxz_r, gyz_u; };
@@ -77,7 +102,7 @@ struct DrTmaCfg2 : DrTmaCfg<TX, TY> {
     static constexpr size_t SMEM2 = (size_t)(END2 + 64) * sizeof(double);
 };
 
-template <int GAVG, int RES, int TX, int TY, bool BND, int PAR>
+template <int GAVG, int RES, int FORM, int TX, int TY, bool BND, int PAR>
 __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, const DrTmaps& T, const DrFusedPtrs& g,
                                             double* sm, unsigned long long* bars, const int s, const int t, const int k,
                                             const int kb, const int ke, const bool store, const int i, const int j,
@@ -106,9 +131,10 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
     const double dzz = (vzn - vzc) * ih;
     const double lam_div = fma(-(2.0 / 3.0), Gc, Kc) * (dxx + dyy + dzz);
     const double g2 = 2.0 * Gc;
-    const double nsxx = (Bs[1 * PL] + th * fma(g2, dxx, lam_div)) * ri;
-    const double nsyy = (Bs[2 * PL] + th * fma(g2, dyy, lam_div)) * ri;
-    const double nszz = (Bs[3 * PL] + th * fma(g2, dzz, lam_div)) * ri;
+    // FORM 0: relaxation toward Hooke's law (Eq. 12-13); FORM 1 (displacement form): Hooke's law itself
+    const double nsxx = FORM ? fma(g2, dxx, lam_div) : (Bs[1 * PL] + th * fma(g2, dxx, lam_div)) * ri;
+    const double nsyy = FORM ? fma(g2, dyy, lam_div) : (Bs[2 * PL] + th * fma(g2, dyy, lam_div)) * ri;
+    const double nszz = FORM ? fma(g2, dzz, lam_div) : (Bs[3 * PL] + th * fma(g2, dzz, lam_div)) * ri;
     const double hc = fma(4.0 / 3.0, Gc, Kc);
     const double gl = Ac[3 * PL - 1], gd = Ac[3 * PL - TX], gld = Ac[3 * PL - TX - 1];
     const double gln = An[3 * PL - 1], gdn = An[3 * PL - TX];
@@ -143,9 +169,9 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
             + dr_dshear(vzn, vzn_d, j, ny, dr_u0(P, 2, x, j == 0 ? 0.0 : P.Ly, (k + 1) * h));
         zyz = false;
     }
-    const double ntxy = zxy ? 0.0 : (Bs[4 * PL] + th * gxy * (exy * ih)) * ri;
-    const double ntxz = zxz ? 0.0 : (Bs[5 * PL] + th * gxz * (exz * ih)) * ri;
-    const double ntyz = zyz ? 0.0 : (Bs[6 * PL] + th * gyz * (eyz * ih)) * ri;
+    const double ntxy = zxy ? 0.0 : (FORM ? gxy * (exy * ih) : (Bs[4 * PL] + th * gxy * (exy * ih)) * ri);
+    const double ntxz = zxz ? 0.0 : (FORM ? gxz * (exz * ih) : (Bs[5 * PL] + th * gxz * (exz * ih)) * ri);
+    const double ntyz = zyz ? 0.0 : (FORM ? gyz * (eyz * ih) : (Bs[6 * PL] + th * gyz * (eyz * ih)) * ri);
 
     X[X_SXX * PL] = nsxx; X[X_SYY * PL] = nsyy; X[X_TXY * PL] = ntxy; X[X_HC * PL] = hc; X[X_GXY * PL] = gxy;
     X[X_TXZ * PL] = ntxz; X[X_TYZ * PL] = ntyz; X[X_GXZ * PL] = gxz; X[X_GYZ * PL] = gyz;
@@ -158,13 +184,7 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
         unsigned long long* bar = bars + (b & 3);
         double* da = sm + Cfg::RING_A + (b & 3) * (DR_TMA_NA * PL);
         double* db = sm + Cfg::RING_B + ((b - 1) % 3) * (DR_TMA_NB * PL);
-        dr_mbar_expect_tx(bar, Cfg::BYTES_A + Cfg::BYTES_B);
-#pragma unroll
-        for (int f = 0; f < DR_TMA_NA; ++f) dr_tma_load_3d(da + f * PL, &T.m[f], bar, x0, y0, m + 1, T.l2_hint);
-#pragma unroll
-        for (int f = 0; f < 5; ++f) dr_tma_load_3d(db + f * PL, &T.m[DR_TMA_NA + f], bar, x0, y0, m, T.l2_hint);
-        dr_tma_load_3d(db + 5 * PL, &T.m[DR_TMA_NA + 5], bar, x0, y0, m + 1, T.l2_hint);
-        dr_tma_load_3d(db + 6 * PL, &T.m[DR_TMA_NA + 6], bar, x0, y0, m + 1, T.l2_hint);
+        dr_tma_issue_batch<FORM, TX, TY>(T, bar, da, db, x0, y0, m, true);
     }
 
     // ================= stage B: new velocities, stores =================
@@ -179,6 +199,7 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
             const bool ci = !BND || i < nx, cj = !BND || j < ny;
             if (ck) {
                 double nvx = vxc, nvy = vyc;
+                double nwx = FORM ? Bs[1 * PL] : 0.0, nwy = FORM ? Bs[2 * PL] : 0.0;     // FORM 1: old w (kept at wall / dead nodes)
                 if (cj) {                           // v_x at (i, j+1/2, k+1/2)
                     if (!BND || (i >= 1 && i <= nx - 1)) {
                         const double Fx = ((nsxx - Xc[X_SXX * PL - 1]) + (Xc[X_TXY * PL + TX] - ntxy) + (ntxz - fc.txz)) * ih;
@@ -186,11 +207,12 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
                         if (Hn > 0.0) {
                             const double rH = dr_rcp(Hn);
                             if (RES) { const double r = fabs(Fx) * rH; rnan |= !(r == r); rmax = dr_max(rmax, r); }
-                            nvx = fma(c2t * rH, Fx, vxc);
+                            if (FORM) { nwx = fma(c2t * th * rH, Fx, (1.0 - th) * nwx); nvx = vxc + nwx; }
+                            else nvx = fma(c2t * rH, Fx, vxc);
                         }
                     }
                     g.o_vx[o] = nvx;
-                    g.o_txz[o] = fc.txz;
+                    if (FORM) g.o_sxx[o] = nwx; else g.o_txz[o] = fc.txz;
                 }
                 if (ci) {                           // v_y at (i+1/2, j, k+1/2)
                     if (!BND || (j >= 1 && j <= ny - 1)) {
@@ -199,36 +221,42 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
                         if (Hn > 0.0) {
                             const double rH = dr_rcp(Hn);
                             if (RES) { const double r = fabs(Fy) * rH; rnan |= !(r == r); rmax = dr_max(rmax, r); }
-                            nvy = fma(c2t * rH, Fy, vyc);
+                            if (FORM) { nwy = fma(c2t * th * rH, Fy, (1.0 - th) * nwy); nvy = vyc + nwy; }
+                            else nvy = fma(c2t * rH, Fy, vyc);
                         }
                     }
                     g.o_vy[o] = nvy;
-                    g.o_tyz[o] = fc.tyz;
+                    if (FORM) g.o_syy[o] = nwy; else g.o_tyz[o] = fc.tyz;
                 }
-                g.o_txy[o] = ntxy;
-                if (ci && cj) { g.o_sxx[o] = nsxx; g.o_syy[o] = nsyy; g.o_szz[o] = nszz; }
-            } else {                                // k == nz: only the top faces
+                if (!FORM) {
+                    g.o_txy[o] = ntxy;
+                    if (ci && cj) { g.o_sxx[o] = nsxx; g.o_syy[o] = nsyy; g.o_szz[o] = nszz; }
+                }
+            } else if (!FORM) {                     // k == nz: only the top faces
                 if (cj) g.o_txz[o] = fc.txz;
                 if (ci) g.o_tyz[o] = fc.tyz;
             }
             if (ci && cj) {                         // v_z at (i+1/2, j+1/2, k)
                 double nvz = vzc;
+                double nwz = FORM ? Bs[3 * PL] : 0.0;
                 if (k >= 1 && k <= nz - 1) {
                     const double Fz = ((fc.txz_r - fc.txz) + (fc.tyz_u - fc.tyz) + (nszz - fc.szz)) * ih;
                     const double Hn = dr_max(dr_max(dr_max(fc.hc, hc), dr_max(fc.gxz, fc.gxz_r)), dr_max(fc.gyz, fc.gyz_u));
                     if (Hn > 0.0) {
                         const double rH = dr_rcp(Hn);
                         if (RES) { const double r = fabs(Fz) * rH; rnan |= !(r == r); rmax = dr_max(rmax, r); }
-                        nvz = fma(c2t * rH, Fz, vzc);
+                        if (FORM) { nwz = fma(c2t * th * rH, Fz, (1.0 - th) * nwz); nvz = vzc + nwz; }
+                        else nvz = fma(c2t * rH, Fz, vzc);
                     }
                 }
                 g.o_vz[o] = nvz;
+                if (FORM) g.o_szz[o] = nwz;
             }
         }
     }
 }
 
-template <int GAVG, int RES, int TX, int TY, bool BND>
+template <int GAVG, int RES, int FORM, int TX, int TY, bool BND>
 __device__ __forceinline__ void dr_tma_march(const DrLayout& L, const DrPT& P, const DrTmaps& T, const DrFusedPtrs& g,
                                              double* sm, unsigned long long* bars, const int s, const int kb, const int ke,
                                              const int i, const int j, const int x0, const int y0,
@@ -238,13 +266,13 @@ __device__ __forceinline__ void dr_tma_march(const DrLayout& L, const DrPT& P, c
     fb = fa;
     int k = kb - 1;
     for (int t = 0; k < ke; t += 2, k += 2) {
-        dr_tma_step<GAVG, RES, TX, TY, BND, 0>(L, P, T, g, sm, bars, s, t, k, kb, ke, k >= kb, i, j, x0, y0, producer, midrow, inner, fa, fb, rmax, rnan);
+        dr_tma_step<GAVG, RES, FORM, TX, TY, BND, 0>(L, P, T, g, sm, bars, s, t, k, kb, ke, k >= kb, i, j, x0, y0, producer, midrow, inner, fa, fb, rmax, rnan);
         if (k + 1 < ke)
-            dr_tma_step<GAVG, RES, TX, TY, BND, 1>(L, P, T, g, sm, bars, s, t + 1, k + 1, kb, ke, true, i, j, x0, y0, producer, midrow, inner, fb, fa, rmax, rnan);
+            dr_tma_step<GAVG, RES, FORM, TX, TY, BND, 1>(L, P, T, g, sm, bars, s, t + 1, k + 1, kb, ke, true, i, j, x0, y0, producer, midrow, inner, fb, fa, rmax, rnan);
     }
 }
 
-template <int GAVG, int RES, int TX, int TY>
+template <int GAVG, int RES, int FORM, int TX, int TY>
 __global__ void __launch_bounds__(TX * TY, 1)
 k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int lz, unsigned long long* res_bits) {
     extern __shared__ __align__(1024) double sm[];
@@ -275,14 +303,8 @@ k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int 
             if (m <= ke) {
                 unsigned long long* bar = bars + b;
                 double* da = sm + Cfg::RING_A + b * (DR_TMA_NA * PL);
-                dr_mbar_expect_tx(bar, b == 0 ? Cfg::BYTES_A : Cfg::BYTES_A + Cfg::BYTES_B);
-                for (int f = 0; f < DR_TMA_NA; ++f) dr_tma_load_3d(da + f * PL, &T.m[f], bar, x0, y0, m + 1, T.l2_hint);
-                if (b >= 1) {
-                    double* db = sm + Cfg::RING_B + (b - 1) * (DR_TMA_NB * PL);
-                    for (int f = 0; f < 5; ++f) dr_tma_load_3d(db + f * PL, &T.m[DR_TMA_NA + f], bar, x0, y0, m, T.l2_hint);
-                    dr_tma_load_3d(db + 5 * PL, &T.m[DR_TMA_NA + 5], bar, x0, y0, m + 1, T.l2_hint);
-                    dr_tma_load_3d(db + 6 * PL, &T.m[DR_TMA_NA + 6], bar, x0, y0, m + 1, T.l2_hint);
-                }
+                double* db = sm + Cfg::RING_B + (b >= 1 ? b - 1 : 0) * (DR_TMA_NB * PL);
+                dr_tma_issue_batch<FORM, TX, TY>(T, bar, da, db, x0, y0, m, b >= 1);
             }
         }
     }
@@ -297,8 +319,8 @@ k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int 
     double rmax = 0.0;
     bool rnan = false;
     const bool interior = i0 >= 2 && i0 + TX - 2 <= nx - 1 && j0 >= 2 && j0 + TY - 2 <= ny - 1;
-    if (interior) dr_tma_march<GAVG, RES, TX, TY, false>(L, P, T, g, sm, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
-    else          dr_tma_march<GAVG, RES, TX, TY, true>(L, P, T, g, sm, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
+    if (interior) dr_tma_march<GAVG, RES, FORM, TX, TY, false>(L, P, T, g, sm, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
+    else          dr_tma_march<GAVG, RES, FORM, TX, TY, true>(L, P, T, g, sm, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
 
     if (RES) {
         __shared__ unsigned long long smr[32];

@@ -42,7 +42,7 @@ def field_errors(o, s, K, G, eps0, h=1.0):
 
 
 def run_pair(oracle_mod, gpu, K, G, lc, eps0, niter, h=1.0, **params):
-    o = oracle_mod.Oracle(K, G, h=h, **{k: v for k, v in params.items() if k != "kernel"})
+    o = oracle_mod.Oracle(K, G, h=h, **{k: v for k, v in params.items() if k not in ("kernel", "zchunk")})
     s = gpu.Solver(to_dev(K), to_dev(G), h=h, **params)
     o.step(lc, eps0, niter)
     s.step(lc, eps0, niter)
@@ -237,3 +237,47 @@ def test_full_size_cfg5_703(oracle_mod, gpu):
     errs, ro, rs, _, _ = run_pair(oracle_mod, gpu, K, G, 2, 1e-4, 3)
     assert max(errs) <= FIELD_TOL, errs
     assert abs(ro - rs) <= 1e-9 * ro
+
+
+# ---------------------------------------------------------------- displacement form (DR_FORM = 1, S: 8(f) f1)
+@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("lc", range(6))
+def test_displacement_form_fields_config1(oracle_mod, gpu, kernel, lc):
+    K, G, _ = inputs.config1_sphere()
+    errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, 1e-4, 100, kernel=kernel, form=1)
+    assert max(errs) <= FIELD_TOL, errs
+    assert abs(ro - rs) <= 1e-9 * ro
+    assert np.max(np.abs(ao - as_)) <= 1e-10 * np.max(np.abs(ao))
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_displacement_form_ragged_void_fluid_and_variants(oracle_mod, gpu, kernel):
+    K, G = inputs.random_smooth((37, 21, 19), seed=77)
+    K[3:6, 4:9, 5:30] = 0.0; G[3:6, 4:9, 5:30] = 0.0          # void
+    G[10:12, 2:6, 3:9] = 0.0                                   # fluid
+    for lc, extra in ((0, {}), (3, dict(bc_mode=1)), (4, dict(gavg=1)), (5, dict(cfl=0.5, st_factor=0.7))):
+        errs, ro, rs, _, _ = run_pair(oracle_mod, gpu, K, G, lc, -2e-3, 30, h=0.5, kernel=kernel, form=1, **extra)
+        assert max(errs) <= FIELD_TOL, (lc, errs)
+        assert abs(ro - rs) <= 1e-9 * ro
+    errs, _, _, ao, as_ = run_pair(oracle_mod, gpu, K, G, 2, 1e-3, 0, kernel=kernel, form=1)      # initial fields
+    assert max(errs) <= 1e-13, errs
+
+
+def test_displacement_form_converged_C_and_continue(oracle_mod, gpu):
+    K, G, _ = inputs.config1_sphere()
+    o = oracle_mod.Oracle(K, G, form=1)
+    Co, logo = o.solve_all(1e-4, 1e-8, 3200)
+    s = gpu.Solver(to_dev(K), to_dev(G), form=1)
+    Cs, logs = s.solve_all(1e-4, 1e-8, 3200)
+    assert [l[1] for l in logo] == [l[1] for l in logs] and all(l[0] == 0 for l in logs)
+    assert np.max(np.abs(Co - Cs)) <= C_TOL * np.max(np.abs(Co))
+    # same fixed point as the paper's stress-relaxation form
+    s0 = gpu.Solver(to_dev(K), to_dev(G))
+    C0, _ = s0.solve_all(1e-4, 1e-8, 3200)
+    assert np.max(np.abs(C0 - Cs)) <= 1e-6 * np.max(np.abs(C0))
+    # step + get_field (forms the stresses) + iterate continues from the same state
+    o.step(2, 1e-4, 30)
+    s.step(2, 1e-4, 10); s.get_field("sxx"); s.iterate(2, 1e-4, 20)
+    import torch
+    torch.cuda.synchronize()
+    assert max(field_errors(o, s, K, G, 1e-4)) <= FIELD_TOL

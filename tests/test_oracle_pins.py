@@ -289,6 +289,25 @@ def test_full_kubc_gives_symmetric_and_stiffer_C(two_phase, oracle_mod):
     assert all(Ck[a, a] >= C[a, a] - 1e-9 for a in range(6))     # more constraint -> stiffer
 
 
+# ---------------------------------------------------------------- P10: displacement form has the same fixed point
+def test_P10_displacement_form_converges_to_the_same_C(two_phase, oracle_mod):
+    K, G, m, C, _ = two_phase
+    o = oracle_mod.Oracle(K, G, form=1)
+    for lc in (0, 2, 4):
+        assert o.solve(lc, 1e-4, 1e-9, 20000) == 0
+        assert np.max(np.abs(o.avg_stress() / 1e-4 - C[:, lc])) <= 2e-7 * C[0, 0]
+
+
+def test_P10b_displacement_form_against_bruteforce(oracle_mod):
+    K, G = inputs.random_smooth((4, 5, 3), seed=11)
+    # theta = C~ St / n_max must stay well below 1 for the explicit damping: on a 5-cell grid scale St down
+    o = oracle_mod.Oracle(K, G, form=1, st_factor=0.4, ncheck=20)
+    C, log = o.solve_all(1e-4, 1e-11, 20000)
+    assert all(l[0] == 0 for l in log)
+    Cb = bruteforce.effective_C(K, G, 1e-4, 1.0, 0)
+    assert np.max(np.abs(C - Cb)) <= 1e-8 * np.max(Cb)
+
+
 # ---------------------------------------------------------------- P13: axis permutation
 def test_P13_cyclic_permutation_of_axes_permutes_C(oracle_mod):
     K, G, _ = inputs.random_two_phase((6, 5, 4), frac=0.3, seed=3)
