@@ -88,6 +88,16 @@ dr_status dr_set_param(dr_handle* h, int id, double value);
  * volume averages (Eq. 7) and column load_case of C* (Eq. 9, 22).  eps0 != 0, tol > 0, maxiter >= 1. */
 dr_status dr_solve(dr_handle* h, int load_case, double eps0, double tol, int maxiter);
 
+/* The six load cases at once on six solvers (h[lc] solves load case lc; six distinct handles, each with its own
+ * workspace and, to overlap on the device, its own stream).  One host thread enqueues every unfinished load case up
+ * to its next residual check before it waits for any of them, so small grids that cannot fill the GPU alone run
+ * concurrently (one direct test per stiffness column).  Same iterates and stopping rule as six dr_solve
+ * calls.  status_out: HOST, 6 ints (dr_status per load case) or NULL.  Returns the worst status. */
+dr_status dr_solve_six(dr_handle* const h[6], double eps0, double tol, int maxiter, int status_out[6]);
+
+/* C* (HOST, row-major out[6*m + n]) with column n taken from h[n], after dr_solve_six. */
+dr_status dr_effective_C_six(dr_handle* const h[6], double out[36]);
+
 /* Same with a fixed iteration count and no convergence test (parity tests): initial fields, niter >= 0
  * iterations, the residual of the last iteration, the volume averages and the (unconverged) column. */
 dr_status dr_step(dr_handle* h, int load_case, double eps0, int niter);

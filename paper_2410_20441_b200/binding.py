@@ -16,7 +16,7 @@ OK, ERR_ARG, ERR_WORKSPACE, ERR_CUDA, ERR_DIVERGED, ERR_STATE, MAXITER = range(7
 CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK, FORM = range(9)
 PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK, form=FORM)
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
-EXPORTS = ("dr_workspace_bytes", "dr_create", "dr_set_param", "dr_solve", "dr_step", "dr_iterate",
+EXPORTS = ("dr_workspace_bytes", "dr_create", "dr_set_param", "dr_solve", "dr_solve_six", "dr_effective_C_six", "dr_step", "dr_iterate",
            "dr_effective_C", "dr_avg_stress", "dr_info", "dr_get_field", "dr_solve_image_host",
            "dr_launch_count", "dr_last_error", "dr_destroy")
 
@@ -38,6 +38,8 @@ def lib():
         L.dr_set_param.argtypes = [vp, C.c_int, C.c_double]
         L.dr_solve.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int]
         L.dr_step.argtypes = [vp, C.c_int, C.c_double, C.c_int]
+        L.dr_solve_six.argtypes = [C.POINTER(vp), C.c_double, C.c_double, C.c_int, C.POINTER(C.c_int)]
+        L.dr_effective_C_six.argtypes = [C.POINTER(vp), dp]
         L.dr_iterate.argtypes = [vp, C.c_int, C.c_double, C.c_int]
         L.dr_effective_C.argtypes = [vp, dp]
         L.dr_avg_stress.argtypes = [vp, dp]
@@ -165,6 +167,31 @@ class Solver:
             self.close()
         except Exception:
             pass
+
+
+def solve_six(K, G, h=1.0, eps0=1e-4, tol=1e-8, maxiter=100000, **params):
+    """dr_solve_six: six Solver handles (own workspace, own torch stream each), load case lc on handle lc.
+    Returns (C[6,6], [(status, iters, residual)]*6, solvers)."""
+    import numpy as np
+    import torch
+    cur = torch.cuda.current_stream(K.device)
+    solvers = []
+    for lc in range(6):
+        st = torch.cuda.Stream(device=K.device)
+        st.wait_stream(cur)
+        solvers.append(Solver(K, G, h=h, stream=st, **params))
+    arr = (C.c_void_p * 6)(*[s._h for s in solvers])
+    stat = (C.c_int * 6)()
+    with torch.cuda.device(K.device):
+        rc = lib().dr_solve_six(arr, eps0, tol, maxiter, stat)
+    if rc not in (OK, MAXITER):
+        raise DrError(rc, "dr_solve_six failed: " + "; ".join(lib().dr_last_error(s._h).decode() for s in solvers))
+    out = np.zeros(36)
+    rc2 = lib().dr_effective_C_six(arr, out.ctypes.data_as(C.POINTER(C.c_double)))
+    if rc2 != OK:
+        raise DrError(rc2, "dr_effective_C_six failed")
+    log = [(stat[lc],) + solvers[lc].info()[:2] for lc in range(6)]
+    return out.reshape(6, 6), log, solvers
 
 
 def solve_image_host(K_host, G_host, h=1.0, eps0=1e-4, tol=1e-8, maxiter=100000, ncheck=0,

@@ -421,6 +421,84 @@ extern "C" dr_status dr_solve(dr_handle* H, int lc, double eps0, double tol, int
     return status;
 }
 
+// SURVEY 8(a) row a7 / north_star (c): the six load cases as six solvers on six streams.  One host thread enqueues, for
+// every unfinished load case, the iterations up to its next residual check (no synchronisation), and only then waits
+// for the six 8-byte residuals; small grids, whose single solve cannot fill the GPU, overlap on the device.
+extern "C" dr_status dr_solve_six(dr_handle* const h[6], double eps0, double tol, int maxiter, int status_out[6]) {
+    if (!h) return DR_ERR_ARG;
+    for (int lc = 0; lc < 6; ++lc) {
+        if (!h[lc]) return DR_ERR_ARG;
+        for (int m = 0; m < lc; ++m) if (h[m] == h[lc]) return fail(h[lc], DR_ERR_ARG, "dr_solve_six needs six distinct handles");
+        if (bad_lc(h[lc], lc, eps0)) return DR_ERR_ARG;
+        if (!(tol > 0.0) || maxiter < 1) return fail(h[lc], DR_ERR_ARG, "bad tol or maxiter");
+    }
+    DrPT P[6];
+    int it[6];
+    bool active[6], pending[6];
+    dr_status st[6];
+    for (int lc = 0; lc < 6; ++lc) {
+        dr_handle* H = h[lc];
+        CK(cudaEventRecord(H->e0, H->st));
+        dr_status s = prepare(H, lc, eps0);
+        if (s != DR_OK) return s;
+        P[lc] = make_pt(H, lc, eps0);
+        it[lc] = 0; active[lc] = true; pending[lc] = false; st[lc] = DR_MAXITER; H->residual = INFINITY;
+    }
+    for (bool any = true; any;) {
+        for (int lc = 0; lc < 6; ++lc) {
+            if (!active[lc]) continue;
+            dr_handle* H = h[lc];
+            const int n = std::min(H->ncheck - it[lc] % H->ncheck, maxiter - it[lc]);
+            bool chk = false;
+            for (int i = 0; i < n; ++i) {
+                ++it[lc];
+                chk = (it[lc] % H->ncheck == 0);
+                if (chk) CK(cudaMemsetAsync(H->res_bits, 0, 8, H->st));
+                dr_status s = iteration(H, P[lc], chk);
+                if (s != DR_OK) return s;
+            }
+            if (chk) CK(cudaMemcpyAsync(H->pinned, H->res_bits, 8, cudaMemcpyDeviceToHost, H->st));
+            pending[lc] = chk;
+        }
+        any = false;
+        for (int lc = 0; lc < 6; ++lc) {
+            if (!active[lc]) continue;
+            dr_handle* H = h[lc];
+            if (pending[lc]) {
+                CK(cudaStreamSynchronize(H->st));
+                double r;
+                std::memcpy(&r, H->pinned, 8);
+                H->residual = r;
+                if (!std::isfinite(r)) { st[lc] = DR_ERR_DIVERGED; active[lc] = false; H->err = "residual is not finite"; }
+                else if (r <= tol) { st[lc] = DR_OK; active[lc] = false; }
+            }
+            if (active[lc] && it[lc] >= maxiter) { active[lc] = false; H->err = "maxiter reached"; }
+            any = any || active[lc];
+        }
+    }
+    dr_status worst = DR_OK;
+    for (int lc = 0; lc < 6; ++lc) {
+        dr_handle* H = h[lc];
+        H->iters = it[lc];
+        if (st[lc] != DR_ERR_DIVERGED) { dr_status s = averages(H, lc, eps0); if (s != DR_OK) return s; }
+        if (status_out) status_out[lc] = (int)st[lc];
+        if (st[lc] == DR_ERR_DIVERGED) worst = DR_ERR_DIVERGED;
+        else if (st[lc] == DR_MAXITER && worst == DR_OK) worst = DR_MAXITER;
+    }
+    return worst;
+}
+
+// effective stiffness from six handles, column lc taken from h[lc] (after dr_solve_six)
+extern "C" dr_status dr_effective_C_six(dr_handle* const h[6], double out[36]) {
+    if (!h || !out) return DR_ERR_ARG;
+    for (int lc = 0; lc < 6; ++lc) {
+        if (!h[lc]) return DR_ERR_ARG;
+        if (!h[lc]->have[lc]) return fail(h[lc], DR_ERR_STATE, "load case not solved on its handle");
+    }
+    for (int m = 0; m < 6; ++m) for (int lc = 0; lc < 6; ++lc) out[6 * m + lc] = h[lc]->Ccol[lc][m];
+    return DR_OK;
+}
+
 extern "C" dr_status dr_step(dr_handle* H, int lc, double eps0, int niter) {
     if (!H) return DR_ERR_ARG;
     if (bad_lc(H, lc, eps0)) return DR_ERR_ARG;

@@ -281,3 +281,19 @@ def test_displacement_form_converged_C_and_continue(oracle_mod, gpu):
     import torch
     torch.cuda.synchronize()
     assert max(field_errors(o, s, K, G, 1e-4)) <= FIELD_TOL
+
+
+def test_solve_six_on_streams_equals_sequential(oracle_mod, gpu):
+    """row a7: six handles on six streams give the same iterates, iteration counts and C as six dr_solve calls"""
+    K, G, _ = inputs.config1_sphere()
+    Kd, Gd = to_dev(K), to_dev(G)
+    Cs, logs = gpu.Solver(Kd, Gd).solve_all(1e-4, 1e-8, 3200)
+    C6, log6, solvers = gpu.solve_six(Kd, Gd, eps0=1e-4, tol=1e-8, maxiter=3200)
+    assert [l[1] for l in log6] == [l[1] for l in logs] and all(l[0] == 0 for l in log6)
+    assert np.array_equal(C6, Cs)                                  # same kernels, same order: bit-identical
+    o = oracle_mod.Oracle(K, G)
+    Co, _ = o.solve_all(1e-4, 1e-8, 3200)
+    assert np.max(np.abs(Co - C6)) <= C_TOL * np.max(np.abs(Co))
+    # soft status and error paths
+    C6b, log6b, _ = gpu.solve_six(Kd, Gd, eps0=1e-4, tol=1e-30, maxiter=120, ncheck=50)
+    assert all(l[0] == gpu.MAXITER and l[1] == 120 for l in log6b)
