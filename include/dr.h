@@ -133,6 +133,12 @@ dr_status dr_solve_image_host(int nx, int ny, int nz, double h,
                               double eps0, double tol, int maxiter, int ncheck,
                               double C_out[36], int iters_out[6]);
 
+/* Compliance (property) contribution tensor of the inclusions, Eq. 23: S* = S1 + phi H, i.e.
+ * H = ((C*)^-1 - (C1)^-1) / phi.  Pure host post-processing of two effective tensors (the image and the matrix-only
+ * run, BASELINE config 2): all pointers HOST, 6x6 row-major, Voigt with engineering shear; 0 < phi <= 1 is the
+ * inclusion volume fraction.  DR_ERR_ARG if an argument is NULL/out of range or a matrix is singular. */
+dr_status dr_contribution_tensor(const double C_eff[36], const double C_matrix[36], double phi, double H_out[36]);
+
 /* Number of kernel launches this handle has issued so far (for bench.py's gpu_launches). */
 long long dr_launch_count(dr_handle* h);
 

@@ -17,7 +17,7 @@ CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK, FORM = range(9)
 PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK, form=FORM)
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
 EXPORTS = ("dr_workspace_bytes", "dr_create", "dr_set_param", "dr_solve", "dr_solve_six", "dr_effective_C_six", "dr_step", "dr_iterate",
-           "dr_effective_C", "dr_avg_stress", "dr_info", "dr_get_field", "dr_solve_image_host",
+           "dr_effective_C", "dr_avg_stress", "dr_info", "dr_get_field", "dr_solve_image_host", "dr_contribution_tensor",
            "dr_launch_count", "dr_last_error", "dr_destroy")
 
 _lib = None
@@ -47,6 +47,7 @@ def lib():
         L.dr_get_field.argtypes = [vp, C.c_int, vp, C.c_size_t]
         L.dr_solve_image_host.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, vp, vp, vp, vp, C.c_size_t, vp,
                                           C.c_double, C.c_double, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
+        L.dr_contribution_tensor.argtypes = [dp, dp, C.c_double, dp]
         L.dr_launch_count.argtypes = [vp]
         L.dr_launch_count.restype = C.c_longlong
         L.dr_last_error.argtypes = [vp]
@@ -167,6 +168,19 @@ class Solver:
             self.close()
         except Exception:
             pass
+
+
+def contribution_tensor(C_eff, C_matrix, phi):
+    """dr_contribution_tensor: H = (inv(C_eff) - inv(C_matrix)) / phi (Eq. 23 of the paper), 6x6 numpy arrays."""
+    import numpy as np
+    a = np.ascontiguousarray(C_eff, dtype=np.float64).reshape(36)
+    b = np.ascontiguousarray(C_matrix, dtype=np.float64).reshape(36)
+    out = np.zeros(36)
+    dp = C.POINTER(C.c_double)
+    st = lib().dr_contribution_tensor(a.ctypes.data_as(dp), b.ctypes.data_as(dp), float(phi), out.ctypes.data_as(dp))
+    if st != OK:
+        raise DrError(st, "dr_contribution_tensor: bad argument or singular matrix")
+    return out.reshape(6, 6)
 
 
 def solve_six(K, G, h=1.0, eps0=1e-4, tol=1e-8, maxiter=100000, **params):

@@ -600,6 +600,36 @@ extern "C" dr_status dr_solve_image_host(int nx, int ny, int nz, double h, const
     return s != DR_OK ? s : worst;
 }
 
+// 6x6 inverse by Gauss-Jordan elimination with partial pivoting (host); false if singular
+static bool invert6(const double* A, double* inv) {
+    double a[6][12];
+    for (int r = 0; r < 6; ++r) for (int c = 0; c < 6; ++c) { a[r][c] = A[6 * r + c]; a[r][6 + c] = (r == c) ? 1.0 : 0.0; }
+    for (int c = 0; c < 6; ++c) {
+        int piv = c;
+        for (int r = c + 1; r < 6; ++r) if (std::fabs(a[r][c]) > std::fabs(a[piv][c])) piv = r;
+        if (!(std::fabs(a[piv][c]) > 0.0) || !std::isfinite(a[piv][c])) return false;
+        if (piv != c) for (int k = 0; k < 12; ++k) std::swap(a[piv][k], a[c][k]);
+        const double d = 1.0 / a[c][c];
+        for (int k = 0; k < 12; ++k) a[c][k] *= d;
+        for (int r = 0; r < 6; ++r) {
+            if (r == c) continue;
+            const double f = a[r][c];
+            if (f != 0.0) for (int k = 0; k < 12; ++k) a[r][k] -= f * a[c][k];
+        }
+    }
+    for (int r = 0; r < 6; ++r) for (int c = 0; c < 6; ++c) inv[6 * r + c] = a[r][6 + c];
+    return true;
+}
+
+// Eq. 23: S* = S1 + phi H  =>  H = ((C*)^-1 - (C1)^-1) / phi, host post-processing of two results
+extern "C" dr_status dr_contribution_tensor(const double C_eff[36], const double C_matrix[36], double phi, double H_out[36]) {
+    if (!C_eff || !C_matrix || !H_out || !(phi > 0.0) || !(phi <= 1.0)) return DR_ERR_ARG;
+    double Se[36], S1[36];
+    if (!invert6(C_eff, Se) || !invert6(C_matrix, S1)) return DR_ERR_ARG;
+    for (int a = 0; a < 36; ++a) H_out[a] = (Se[a] - S1[a]) / phi;
+    return DR_OK;
+}
+
 extern "C" long long dr_launch_count(dr_handle* H) { return H ? H->launches : 0; }
 
 extern "C" const char* dr_last_error(dr_handle* H) { return H ? H->err.c_str() : "null handle"; }

@@ -297,3 +297,26 @@ def test_solve_six_on_streams_equals_sequential(oracle_mod, gpu):
     # soft status and error paths
     C6b, log6b, _ = gpu.solve_six(Kd, Gd, eps0=1e-4, tol=1e-30, maxiter=120, ncheck=50)
     assert all(l[0] == gpu.MAXITER and l[1] == 120 for l in log6b)
+
+
+def test_cfg2_spheroid_tetragonal_C_and_contribution_tensor(gpu):
+    """BASELINE config 2 at full size: anisotropic C_eff and the property-contribution tensor against the matrix-only
+    result (Eq. 23).  Properties that hold at any size: tetragonal symmetry about z, H positive and largest
+    normal to the oblate inclusion."""
+    K, G, m = inputs.config2_spheroid()
+    s = gpu.Solver(to_dev(K), to_dev(G), ncheck=100)
+    C, log = s.solve_all(1e-4, 1e-8, 19100)
+    assert all(l[0] == 0 for l in log), log
+    s0 = C[0, 0]
+    assert abs(C[0, 0] - C[1, 1]) <= 1e-9 * s0 and abs(C[0, 2] - C[1, 2]) <= 1e-9 * s0 and abs(C[3, 3] - C[4, 4]) <= 1e-9 * s0
+    assert C[2, 2] < C[0, 0] and C[3, 3] < C[5, 5]
+    s.close()
+    # matrix-only run = Hooke (pin P1), solved on the GPU as the config asks
+    K1, G1 = inputs.homogeneous(191, 70.2, 29.0)
+    s1 = gpu.Solver(to_dev(K1), to_dev(G1), ncheck=100)
+    C1, log1 = s1.solve_all(1e-4, 1e-8, 19100)
+    assert all(l[0] == 0 and l[1] == 100 for l in log1)
+    H = gpu.contribution_tensor(C, C1, float(m.mean()))
+    assert all(H[a, a] > 0 for a in range(6))
+    assert H[2, 2] > 5 * H[0, 0] and H[3, 3] > 2 * H[5, 5]           # compliant across the thin direction
+    assert abs(H[0, 0] - H[1, 1]) <= 1e-6 * H[2, 2] and abs(H[3, 3] - H[4, 4]) <= 1e-6 * H[3, 3]

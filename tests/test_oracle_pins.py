@@ -174,6 +174,18 @@ def test_P14_config1_matches_independent_survey_probe(config1_C):
     assert all(5 * 32 <= l[1] <= 20 * 32 for l in log)
 
 
+def test_P14b_sphere_r10_64_matches_independent_survey_probe(oracle_mod):
+    g = read_golden("survey_probe_B.txt")["B6_sphere_r10_64"]
+    K, G, m = inputs.config1_sphere(n=64, r=10.0)
+    o = oracle_mod.Oracle(K, G)
+    assert o.solve(0, 1e-4, 1e-8, 6400) == 0
+    c0, it0 = o.avg_stress() / 1e-4, o.info()[0]
+    assert o.solve(3, 1e-4, 1e-8, 6400) == 0
+    c3, it3 = o.avg_stress() / 1e-4, o.info()[0]
+    assert abs(c0[0] - g[0]) <= 1e-6 * g[0] and abs(c0[1] - g[1]) <= 1e-6 * g[0] and abs(c3[3] - g[2]) <= 1e-6 * g[0]
+    assert (it0, it3) == (int(g[3]), int(g[4]))
+
+
 def dilute_pore(K, G, phi):
     """Eshelby (1957) / Mackenzie dilute spherical pores (special case of Eq. 23, 30-34 P:191)"""
     nu = (3 * K - 2 * G) / (2 * (3 * K + G))
