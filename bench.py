@@ -179,6 +179,7 @@ def main():
     ap.add_argument("--eps0", type=float, default=1e-4)
     ap.add_argument("--ncheck", type=int, default=100)
     ap.add_argument("--kernel", type=int, default=0, help="0 fused with TMA staging (default), 1 split baseline, 2 fused with LDG prefetch")
+    ap.add_argument("--form", type=int, default=0, help="0 stress-relaxation form of the paper (default, 160 B/voxel), 1 displacement form (112 B/voxel)")
     ap.add_argument("--cpu-sample-n", type=int, default=191)
     ap.add_argument("--cpu-iters", type=int, default=100)
     ap.add_argument("--cpu-iters-per-step", type=int, default=5)
@@ -214,7 +215,7 @@ def main():
     lc = shard.load_case_of_rank(rank, world, args.lc)
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
-        s = binding.Solver(Kd, Gd, stream=stream, ncheck=args.ncheck, kernel=args.kernel)
+        s = binding.Solver(Kd, Gd, stream=stream, ncheck=args.ncheck, kernel=args.kernel, form=args.form)
 
         def barrier():
             torch.cuda.synchronize(dev)
@@ -274,7 +275,7 @@ def main():
             del stage, Kh, Gh
             # the solver's workspace was reused by the e2e call: rebuild the handle state
             s.close()
-            s = binding.Solver(Kd, Gd, stream=stream, workspace=s.workspace, ncheck=args.ncheck, kernel=args.kernel)
+            s = binding.Solver(Kd, Gd, stream=stream, workspace=s.workspace, ncheck=args.ncheck, kernel=args.kernel, form=args.form)
 
         tts = None
         if args.time_to_solution and rank == 0:
@@ -287,15 +288,16 @@ def main():
                    "C": [[float("%.6f" % v) for v in row] for row in C]}
 
     peak, peak_src = measured_peak()
+    bpv = 112.0 if args.form == 1 else BYTES_PER_VOXEL_ITER      # algorithmic bytes per voxel-iteration of the form
     value = shard.job_throughput(N, args.steps, world, ms)
-    teff = BYTES_PER_VOXEL_ITER * N * args.steps / (ms * 1e-3) / 1e9
-    kern_gbs = BYTES_PER_VOXEL_ITER * N / (kms * 1e-3) / 1e9
+    teff = bpv * N * args.steps / (ms * 1e-3) / 1e9
+    kern_gbs = bpv * N / (kms * 1e-3) / 1e9
     line = {
         "metric": "pt_voxel_updates_per_s", "value": value, "unit": "voxel-updates/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s: %s" % (args.workload, WORKLOADS[args.workload]["desc"]), "grid": [n, n, n],
-                   "load_case": lc, "ncheck": args.ncheck, "kernel": {0: "fused+TMA", 1: "split", 2: "fused+LDG"}[args.kernel],
+                   "load_case": lc, "ncheck": args.ncheck, "form": "stress-relaxation (paper, 160 B/voxel-iteration)" if args.form == 0 else "displacement (112 B/voxel-iteration)", "kernel": {0: "fused+TMA", 1: "split", 2: "fused+LDG"}[args.kernel],
                    "parallelism": "load cases sharded over %d GPU(s), no collective" % world,
                    "l2": "inputs (%.1f GB per iteration) larger than L2; no flush needed" % (BYTES_PER_VOXEL_ITER * N / 1e9)},
         "T_eff_GBs": teff, "T_eff_frac_of_measured_peak": teff / peak, "T_eff_frac_of_8000_nominal": teff / 8000.0,
@@ -304,8 +306,8 @@ def main():
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": {0: "k_pt_tma", 1: "k_stress_split+k_velocity_split", 2: "k_pt_fused"}[args.kernel],
                      "achieved": kern_gbs, "peak": peak, "unit": "GB/s", "frac": kern_gbs / peak,
-                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.kernel)) if args.n is None else None, "peak_source": peak_src, "launch_ms": kms,
-                     "algorithmic_bytes_per_launch": BYTES_PER_VOXEL_ITER * N},
+                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.kernel)) if (args.n is None and args.form == 0) else None, "peak_source": peak_src, "launch_ms": kms,
+                     "algorithmic_bytes_per_launch": bpv * N},
     }
     if tts is not None:
         line["time_to_full_C"] = tts

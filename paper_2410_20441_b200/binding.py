@@ -10,7 +10,7 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libdr.so")
+LIB_PATH = os.environ.get("DR_LIB") or os.path.join(_HERE, "libdr.so")     # DR_LIB: an alternative build (A/B timing)
 
 OK, ERR_ARG, ERR_WORKSPACE, ERR_CUDA, ERR_DIVERGED, ERR_STATE, MAXITER = range(7)
 CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK, FORM = range(9)
@@ -38,8 +38,9 @@ def lib():
         L.dr_set_param.argtypes = [vp, C.c_int, C.c_double]
         L.dr_solve.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int]
         L.dr_step.argtypes = [vp, C.c_int, C.c_double, C.c_int]
-        L.dr_solve_six.argtypes = [C.POINTER(vp), C.c_double, C.c_double, C.c_int, C.POINTER(C.c_int)]
-        L.dr_effective_C_six.argtypes = [C.POINTER(vp), dp]
+        if hasattr(L, "dr_solve_six"):          # absent only in older builds loaded through DR_LIB for A/B timing
+            L.dr_solve_six.argtypes = [C.POINTER(vp), C.c_double, C.c_double, C.c_int, C.POINTER(C.c_int)]
+            L.dr_effective_C_six.argtypes = [C.POINTER(vp), dp]
         L.dr_iterate.argtypes = [vp, C.c_int, C.c_double, C.c_int]
         L.dr_effective_C.argtypes = [vp, dp]
         L.dr_avg_stress.argtypes = [vp, dp]
@@ -47,7 +48,8 @@ def lib():
         L.dr_get_field.argtypes = [vp, C.c_int, vp, C.c_size_t]
         L.dr_solve_image_host.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, vp, vp, vp, vp, C.c_size_t, vp,
                                           C.c_double, C.c_double, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
-        L.dr_contribution_tensor.argtypes = [dp, dp, C.c_double, dp]
+        if hasattr(L, "dr_contribution_tensor"):
+            L.dr_contribution_tensor.argtypes = [dp, dp, C.c_double, dp]
         L.dr_launch_count.argtypes = [vp]
         L.dr_launch_count.restype = C.c_longlong
         L.dr_last_error.argtypes = [vp]
