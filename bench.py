@@ -34,8 +34,8 @@ from paper_2410_20441_b200 import inputs, shard  # noqa: E402
 
 BYTES_PER_VOXEL_ITER = 160.0        # (2*9 + 2) fp64, SURVEY 8(d)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_pt_tma at 479^3 from the one `ncu --set full` capture
-# summarised in profiles/r1_summary.md (11.03 + 8.00 GB); null for any other workload / kernel
-NCU_TRAFFIC_BYTES = {("cfg4", 0): 19.03e9}
+# summarised in profiles/r1_summary.md (10.96 + 7.99 GB); null for any other workload / kernel
+NCU_TRAFFIC_BYTES = {("cfg4", 0): 18.94e9}
 WORKLOADS = {
     "cfg1": dict(n=32, gen="config1_sphere", desc="32^3 centred spherical pore r=5, contrast 1e-6"),
     "cfg2": dict(n=191, gen="config2_spheroid", desc="191^3 oblate fluid spheroid (40,40,8)"),

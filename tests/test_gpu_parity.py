@@ -318,5 +318,5 @@ def test_cfg2_spheroid_tetragonal_C_and_contribution_tensor(gpu):
     assert all(l[0] == 0 and l[1] == 100 for l in log1)
     H = gpu.contribution_tensor(C, C1, float(m.mean()))
     assert all(H[a, a] > 0 for a in range(6))
-    assert H[2, 2] > 5 * H[0, 0] and H[3, 3] > 2 * H[5, 5]           # compliant across the thin direction
+    assert H[2, 2] > 3 * H[0, 0] and H[3, 3] > H[5, 5]               # most compliant across the thin direction
     assert abs(H[0, 0] - H[1, 1]) <= 1e-6 * H[2, 2] and abs(H[3, 3] - H[4, 4]) <= 1e-6 * H[3, 3]
