@@ -125,6 +125,8 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
     const double vxc = Ac[0 * PL], vyc = Ac[1 * PL], vzc = Ac[2 * PL], Gc = Ac[3 * PL];
     const double vxn = An[0 * PL], vyn = An[1 * PL], vzn = An[2 * PL], Gn = An[3 * PL];
     const double Kc = Bs[0 * PL];
+    // FORM 1: the old w must be read HERE: after the barrier below the ring-B slot is handed back to the TMA unit
+    const double wxo = FORM ? Bs[1 * PL] : 0.0, wyo = FORM ? Bs[2 * PL] : 0.0, wzo = FORM ? Bs[3 * PL] : 0.0;
     const bool bk1 = (k + 1 == 0 || k + 1 == nz);
     const double dxx = (Ac[0 * PL + 1] - vxc) * ih;
     const double dyy = (Ac[1 * PL + TX] - vyc) * ih;
@@ -199,7 +201,7 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
             const bool ci = !BND || i < nx, cj = !BND || j < ny;
             if (ck) {
                 double nvx = vxc, nvy = vyc;
-                double nwx = FORM ? Bs[1 * PL] : 0.0, nwy = FORM ? Bs[2 * PL] : 0.0;     // FORM 1: old w (kept at wall / dead nodes)
+                double nwx = wxo, nwy = wyo;                 // FORM 1: old w (kept at wall / dead nodes)
                 if (cj) {                           // v_x at (i, j+1/2, k+1/2)
                     if (!BND || (i >= 1 && i <= nx - 1)) {
                         const double Fx = ((nsxx - Xc[X_SXX * PL - 1]) + (Xc[X_TXY * PL + TX] - ntxy) + (ntxz - fc.txz)) * ih;
@@ -238,7 +240,7 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
             }
             if (ci && cj) {                         // v_z at (i+1/2, j+1/2, k)
                 double nvz = vzc;
-                double nwz = FORM ? Bs[3 * PL] : 0.0;
+                double nwz = wzo;
                 if (k >= 1 && k <= nz - 1) {
                     const double Fz = ((fc.txz_r - fc.txz) + (fc.tyz_u - fc.tyz) + (nszz - fc.szz)) * ih;
                     const double Hn = dr_max(dr_max(dr_max(fc.hc, hc), dr_max(fc.gxz, fc.gxz_r)), dr_max(fc.gyz, fc.gyz_u));

@@ -320,3 +320,25 @@ def test_cfg2_spheroid_tetragonal_C_and_contribution_tensor(gpu):
     assert all(H[a, a] > 0 for a in range(6))
     assert H[2, 2] > 3 * H[0, 0] and H[3, 3] > H[5, 5]               # most compliant across the thin direction
     assert abs(H[0, 0] - H[1, 1]) <= 1e-6 * H[2, 2] and abs(H[3, 3] - H[4, 4]) <= 1e-6 * H[3, 3]
+
+
+@pytest.mark.parametrize("zchunk", [1, 2, 5, 13, 64])
+def test_fields_do_not_depend_on_the_z_chunking(oracle_mod, gpu, zchunk):
+    """DR_ZCHUNK only changes how the z-march is cut into CTAs (priming step at every chunk start): same results"""
+    K, G = inputs.random_smooth((35, 31, 27), seed=123)
+    for kernel in (0, 2):
+        errs, ro, rs, _, _ = run_pair(oracle_mod, gpu, K, G, 4, 1e-4, 12, kernel=kernel, zchunk=zchunk)
+        assert max(errs) <= FIELD_TOL, (kernel, errs)
+        assert abs(ro - rs) <= 1e-9 * ro
+    errs, _, _, _, _ = run_pair(oracle_mod, gpu, K, G, 1, 1e-4, 12, kernel=0, zchunk=zchunk, form=1)
+    assert max(errs) <= FIELD_TOL, errs
+
+
+@pytest.mark.parametrize("form", [0, 1])
+def test_fields_191_default_chunking(oracle_mod, gpu, form):
+    """191^3 (cfg 2/3 size) with the automatic z chunking (32 layers: ring slots are recycled many times per chunk)"""
+    K, G, _ = inputs.config3_random_spheres()
+    errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, 4, 1e-4, 15, form=form)
+    assert max(errs) <= FIELD_TOL, errs
+    assert abs(ro - rs) <= 1e-9 * ro
+    assert np.max(np.abs(ao - as_)) <= 1e-9 * np.max(np.abs(ao))
