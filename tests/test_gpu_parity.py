@@ -342,3 +342,33 @@ def test_fields_191_default_chunking(oracle_mod, gpu, form):
     assert max(errs) <= FIELD_TOL, errs
     assert abs(ro - rs) <= 1e-9 * ro
     assert np.max(np.abs(ao - as_)) <= 1e-9 * np.max(np.abs(ao))
+
+
+def _fuzz_case(rng):
+    shape = tuple(int(v) for v in rng.integers(2, 70, size=3))
+    kernel = int(rng.integers(0, 3))
+    form = int(rng.integers(0, 2)) if kernel != 2 else 0
+    params = dict(kernel=kernel, form=form, bc_mode=int(rng.integers(0, 2)), gavg=int(rng.integers(0, 2)))
+    if kernel != 1 and rng.uniform() < 0.6:
+        params["zchunk"] = int(rng.integers(1, 40))
+    if rng.uniform() < 0.3:
+        params["st_factor"] = float(rng.uniform(0.5, 0.9))
+    return shape, params, int(rng.integers(0, 6)), float(rng.choice([1e-4, -3e-3])), int(rng.integers(1, 16)), float(rng.choice([1.0, 0.37, 2.5]))
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_fuzz_random_shapes_and_parameters(oracle_mod, gpu, seed):
+    """seeded random shapes (2..69 per axis), kernels, forms, boundary modes, chunkings, void/fluid cells"""
+    rng = np.random.default_rng(1000 + seed)
+    shape, params, lc, eps0, niter, h = _fuzz_case(rng)
+    K, G = inputs.random_smooth(shape, seed=seed)
+    m = rng.uniform(size=K.shape)
+    K[m < 0.05] = 0.0; G[m < 0.05] = 0.0          # void
+    G[(m > 0.05) & (m < 0.1)] = 0.0               # fluid
+    if params.get("form") == 1:
+        params.setdefault("st_factor", 0.5 if max(shape) < 12 else 1.0)      # keep theta well below 1 on tiny grids
+        if max(shape) < 12:
+            params["st_factor"] = 0.4
+    errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, eps0, niter, h=h, **params)
+    assert max(errs) <= FIELD_TOL, (shape, params, lc, niter, errs)
+    assert np.isfinite(rs) and abs(ro - rs) <= 1e-9 * max(ro, 1e-300), (shape, params, ro, rs)
