@@ -118,8 +118,7 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
     const double* Bs = sm + Cfg::RING_B + (t % 3) * (DR_TMA_NB * PL) + s;          // set k+1
     double* X = sm + Cfg::XCH + PAR * (X_COUNT * PL) + s;                           // this step's exchange planes
 
-    // ---- batch t+1 (layer k+1, set k+1) must have landed
-    dr_mbar_wait(bars + ((t + 1) & 3), ((t + 1) >> 2) & 1);
+    // batch t+1 (layer k+1, set k+1) has landed: it was waited for behind the barrier of the previous step
 
     // ================= stage A: new stresses =================
     const double vxc = Ac[0 * PL], vyc = Ac[1 * PL], vzc = Ac[2 * PL], Gc = Ac[3 * PL];
@@ -188,6 +187,9 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
         double* db = sm + Cfg::RING_B + ((b - 1) % 3) * (DR_TMA_NB * PL);
         dr_tma_issue_batch<FORM, TX, TY>(T, bar, da, db, x0, y0, m, true);
     }
+    // ---- wait HERE for the batch of the next step (issued two steps ago), not at the top of the next step: stage B
+    // below and stage A of the next step then form one straight-line region that the scheduler can interleave
+    if (k + 2 <= ke) dr_mbar_wait(bars + ((t + 2) & 3), ((t + 2) >> 2) & 1);
 
     // ================= stage B: new velocities, stores =================
     if (midrow) {
@@ -312,6 +314,7 @@ k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int 
     }
     __syncthreads();                                          // barrier init visible to every waiter
     dr_mbar_wait(bars + 0, 0);                                // layer kb-1
+    dr_mbar_wait(bars + 1, 0);                                // layer kb and set kb (first step)
 
     const long long qcol = L.origin + min(i, nx + 1) + L.sy * min(j, ny + 1);
     DrFusedPtrs g;
