@@ -59,6 +59,9 @@ typedef enum {
     DR_KERNEL = 6,     /* 0 fused z-march kernel with TMA staging [default]; 1 split stress/velocity kernels
                           (baseline); 2 fused z-march kernel with register-prefetched LDG loads              */
     DR_ZCHUNK = 7,     /* z layers per CTA of the fused kernels; 0 = automatic [default] (tuning knob)            */
+    DR_PALETTE = 9,    /* 1 [default]: images with <= 256 distinct (K,G) pairs run the fused kernel on a uint8 phase id
+                          per cell and a 256-entry table instead of the two fp64 modulus fields (same values, 14 B less
+                          HBM traffic per voxel-iteration); 0: always the fp64 modulus fields                        */
     DR_FORM = 8        /* 0 stress-relaxation form of the paper, Eq. 11-13 [default]; 1 displacement form: state u, w,
                           w <- (1-theta) w + C~^2 h^2 F(u)/H_node, u <- u + w, stresses formed on the fly (same fixed
                           point, 112 instead of 160 B per voxel-iteration; DR_KERNEL 0 or 1).  Setting DR_FORM also resets
@@ -138,6 +141,10 @@ dr_status dr_solve_image_host(int nx, int ny, int nz, double h,
  * run, BASELINE config 2): all pointers HOST, 6x6 row-major, Voigt with engineering shear; 0 < phi <= 1 is the
  * inclusion volume fraction.  DR_ERR_ARG if an argument is NULL/out of range or a matrix is singular. */
 dr_status dr_contribution_tensor(const double C_eff[36], const double C_matrix[36], double phi, double H_out[36]);
+
+/* 1 if dr_solve / dr_step on this handle run the phase-id (palette) variant of the fused kernel (the image has at
+ * most 256 distinct (K,G) pairs, DR_PALETTE = 1, DR_KERNEL = 0), else 0. */
+int dr_uses_palette(dr_handle* h);
 
 /* Number of kernel launches this handle has issued so far (for bench.py's gpu_launches). */
 long long dr_launch_count(dr_handle* h);

@@ -13,12 +13,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("DR_LIB") or os.path.join(_HERE, "libdr.so")     # DR_LIB: an alternative build (A/B timing)
 
 OK, ERR_ARG, ERR_WORKSPACE, ERR_CUDA, ERR_DIVERGED, ERR_STATE, MAXITER = range(7)
-CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK, FORM = range(9)
-PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK, form=FORM)
+CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK, FORM, PALETTE = range(10)
+PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK, form=FORM, palette=PALETTE)
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
 EXPORTS = ("dr_workspace_bytes", "dr_create", "dr_set_param", "dr_solve", "dr_solve_six", "dr_effective_C_six", "dr_step", "dr_iterate",
            "dr_effective_C", "dr_avg_stress", "dr_info", "dr_get_field", "dr_solve_image_host", "dr_contribution_tensor",
-           "dr_launch_count", "dr_last_error", "dr_destroy")
+           "dr_uses_palette", "dr_launch_count", "dr_last_error", "dr_destroy")
 
 _lib = None
 
@@ -50,6 +50,8 @@ def lib():
                                           C.c_double, C.c_double, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
         if hasattr(L, "dr_contribution_tensor"):
             L.dr_contribution_tensor.argtypes = [dp, dp, C.c_double, dp]
+        if hasattr(L, "dr_uses_palette"):
+            L.dr_uses_palette.argtypes = [vp]
         L.dr_launch_count.argtypes = [vp]
         L.dr_launch_count.restype = C.c_longlong
         L.dr_last_error.argtypes = [vp]
@@ -148,6 +150,9 @@ class Solver:
         out = self._torch.empty(field_shape(self.nx, self.ny, self.nz, f), dtype=self._torch.float64, device=self.device)
         self._check(lib().dr_get_field(self._h, f, out.data_ptr(), out.numel()))
         return out
+
+    def uses_palette(self):
+        return bool(lib().dr_uses_palette(self._h))
 
     def launch_count(self):
         return lib().dr_launch_count(self._h)

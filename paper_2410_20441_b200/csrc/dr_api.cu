@@ -16,8 +16,10 @@
 #include "dr_kernels_fused.cuh"
 #include "dr_kernels_tma.cuh"
 
+#ifndef FUSED_TX
 #define FUSED_TX 32
 #define FUSED_TY 16
+#endif
 
 struct dr_handle {
     DrLayout L;
@@ -30,6 +32,12 @@ struct dr_handle {
     double* avg_dev;            // 6
     unsigned long long* res_bits;
     unsigned long long* hmax_bits;
+    unsigned char* ids;         // uint8 phase id per cell on the padded box (palette path)
+    unsigned long long *palK, *palG;   // palette keys (bit patterns), 256 each
+    double* pal;                // palette values K[256], G[256] after the void clamp
+    bool has_pal;               // the image has at most 256 distinct (K,G) pairs
+    int use_pal;                // DR_PALETTE
+    CUtensorMap tm_ids;
     unsigned int* flags;
     // host
     double* pinned;             // 8 doubles, page-locked
@@ -81,12 +89,13 @@ static bool sizes_ok(int nx, int ny, int nz) {
 
 static size_t field_bytes(const DrLayout& L) { return align_up((size_t)L.count * sizeof(double), 256); }
 static const int N_BIG = 2 * F_COUNT + 4;        // 18 state fields + K0, G0, K, G
-static const size_t SMALL_BYTES = align_up((size_t)DR_AVG_BLOCKS * 6 * sizeof(double), 256) + 1024;
+static const size_t SMALL_BYTES = align_up((size_t)DR_AVG_BLOCKS * 6 * sizeof(double), 256) + 1024 + 3 * 4096;   // + palette keys and values
+static size_t ids_bytes(const DrLayout& L) { return align_up((size_t)L.count, 256); }
 
 extern "C" size_t dr_workspace_bytes(int nx, int ny, int nz) {
     if (!sizes_ok(nx, ny, nz)) return 0;
     DrLayout L = dr_make_layout(nx, ny, nz);
-    return (size_t)N_BIG * field_bytes(L) + SMALL_BYTES;
+    return (size_t)N_BIG * field_bytes(L) + ids_bytes(L) + SMALL_BYTES;
 }
 
 // z-chunk length of the fused kernels: make the CTA count fill whole waves of 148 SMs while keeping the priming
@@ -128,6 +137,18 @@ static bool make_tmap(dr_handle* H, dr_encode_fn enc, CUtensorMap* out, double* 
     return true;
 }
 
+static bool make_ids_tmap(dr_handle* H, dr_encode_fn enc) {
+    const DrLayout& L = H->L;
+    cuuint64_t dims[3] = {(cuuint64_t)L.PX, (cuuint64_t)L.PY, (cuuint64_t)L.PZ};
+    cuuint64_t strides[2] = {(cuuint64_t)L.PX, (cuuint64_t)L.PX * L.PY};          // bytes; PX is a multiple of 16
+    cuuint32_t box[3] = {DR_ID_ROW, FUSED_TY, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(&H->tm_ids, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, H->ids, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { H->err = "cuTensorMapEncodeTiled(ids) failed (" + std::to_string((int)r) + ")"; return false; }
+    return true;
+}
+
 static bool make_all_tmaps(dr_handle* H) {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qr;
@@ -137,7 +158,7 @@ static bool make_all_tmaps(dr_handle* H) {
     }
     dr_encode_fn enc = (dr_encode_fn)fn;
     for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) if (!make_tmap(H, enc, &H->tm_state[b][f], H->buf[b][f])) return false;
-    return make_tmap(H, enc, &H->tm_K, H->K) && make_tmap(H, enc, &H->tm_G, H->G);
+    return make_tmap(H, enc, &H->tm_K, H->K) && make_tmap(H, enc, &H->tm_G, H->G) && make_ids_tmap(H, enc);
 }
 
 extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K, const double* G,
@@ -162,6 +183,11 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
     H->res_bits = (unsigned long long*)p; p += 256;
     H->hmax_bits = (unsigned long long*)p; p += 256;
     H->flags = (unsigned int*)p; p += 256;
+    H->palK = (unsigned long long*)p; p += 2048; H->palG = (unsigned long long*)p; p += 2048;
+    H->pal = (double*)p; p += 4096;
+    p = (char*)align_up((size_t)p, 256);
+    H->ids = (unsigned char*)p; p += ids_bytes(H->L);
+    H->has_pal = false; H->use_pal = 1;
     H->pinned = nullptr; H->e0 = H->e1 = nullptr;
     H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->kernel = 0; H->form = 0;
     H->void_applied = 0.0; H->hmax = 0.0;
@@ -175,7 +201,8 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
         if (!cuda_ok(H, cudaMallocHost((void**)&H->pinned, 8 * sizeof(double)), "cudaMallocHost")) { st = DR_ERR_CUDA; break; }
         if (!cuda_ok(H, cudaEventCreate(&H->e0), "cudaEventCreate") || !cuda_ok(H, cudaEventCreate(&H->e1), "cudaEventCreate")) { st = DR_ERR_CUDA; break; }
         // state fields and moduli boxes start as zeros (halo nodes are never written afterwards)
-        if (!cuda_ok(H, cudaMemsetAsync(workspace, 0, (size_t)N_BIG * fb + SMALL_BYTES, H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }
+        if (!cuda_ok(H, cudaMemsetAsync(workspace, 0, dr_workspace_bytes(nx, ny, nz), H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }
+        if (!cuda_ok(H, cudaMemsetAsync(H->palK, 0xff, 4096, H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }     // palK and palG := EMPTY
         dim3 blk(64, 4, 1), grd((nx + 2 + 63) / 64, (ny + 2 + 3) / 4, nz + 2);
         k_pad_moduli<<<grd, blk, 0, H->st>>>(H->L, K, G, H->K0, H->G0, H->flags, H->hmax_bits);
         H->launches++;
@@ -184,11 +211,28 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
         k_void_clamp<<<(unsigned)((cnt + 255) / 256), 256, 0, H->st>>>(H->L, H->K0, H->G0, H->K, H->G, 0.0);
         H->launches++;
         if (!cuda_ok(H, cudaGetLastError(), "k_void_clamp")) { st = DR_ERR_CUDA; break; }
+        // palette of the distinct (K,G) pairs; more than 256 of them (flag 2) simply leaves the fp64 path in charge
+        {
+            const long long Ncell = (long long)nx * ny * nz;
+            k_pal_build<<<(unsigned)((Ncell + 255) / 256), 256, 0, H->st>>>(Ncell, K, G, H->palK, H->palG, H->flags);
+            H->launches++;
+            if (!cuda_ok(H, cudaGetLastError(), "k_pal_build")) { st = DR_ERR_CUDA; break; }
+        }
         unsigned long long hb = 0; unsigned int fl = 0;
         if (!cuda_ok(H, cudaMemcpyAsync(&hb, H->hmax_bits, 8, cudaMemcpyDeviceToHost, H->st), "memcpy") ||
             !cuda_ok(H, cudaMemcpyAsync(&fl, H->flags, 4, cudaMemcpyDeviceToHost, H->st), "memcpy") ||
             !cuda_ok(H, cudaStreamSynchronize(H->st), "cudaStreamSynchronize")) { st = DR_ERR_CUDA; break; }
-        if (fl) { st = DR_ERR_ARG; break; }
+        if (fl & 1u) { st = DR_ERR_ARG; break; }
+        if (!(fl & 2u)) {
+            k_pal_assign<<<grd, blk, 0, H->st>>>(H->L, K, G, H->palK, H->palG, H->ids, H->flags);
+            k_pal_values<<<1, 256, 0, H->st>>>(H->palK, H->palG, H->pal, 0.0);
+            H->launches += 2;
+            unsigned int fl2 = 0;
+            if (!cuda_ok(H, cudaGetLastError(), "k_pal_assign") ||
+                !cuda_ok(H, cudaMemcpyAsync(&fl2, H->flags, 4, cudaMemcpyDeviceToHost, H->st), "memcpy") ||
+                !cuda_ok(H, cudaStreamSynchronize(H->st), "cudaStreamSynchronize")) { st = DR_ERR_CUDA; break; }
+            H->has_pal = !(fl2 & 4u);
+        }
         std::memcpy(&H->hmax, &hb, 8);
         // opt in to the large dynamic shared memory of the fused kernel (all instantiations)
         const int smem = (int)DrFusedCfg<FUSED_TX, FUSED_TY>::SMEM;
@@ -198,8 +242,9 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (!cuda_ok(H, e, "cudaFuncSetAttribute")) { st = DR_ERR_CUDA; break; }
-        const int smem_t = (int)DrTmaCfg2<FUSED_TX, FUSED_TY>::SMEM2;
-#define DR_SET_TMA_ATTR(G_, R_, F_) if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<G_, R_, F_, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t)
+        const int smem_t = (int)DrTmaCfg2<FUSED_TX, FUSED_TY, 0>::SMEM2, smem_p = (int)DrTmaCfg2<FUSED_TX, FUSED_TY, 1>::SMEM2;
+#define DR_SET_TMA_ATTR(G_, R_, F_) if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<G_, R_, F_, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t); \
+                                    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<G_, R_, F_, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_p)
         DR_SET_TMA_ATTR(0, 0, 0); DR_SET_TMA_ATTR(0, 1, 0); DR_SET_TMA_ATTR(1, 0, 0); DR_SET_TMA_ATTR(1, 1, 0);
         DR_SET_TMA_ATTR(0, 0, 1); DR_SET_TMA_ATTR(0, 1, 1); DR_SET_TMA_ATTR(1, 0, 1); DR_SET_TMA_ATTR(1, 1, 1);
 #undef DR_SET_TMA_ATTR
@@ -230,6 +275,7 @@ extern "C" dr_status dr_set_param(dr_handle* H, int id, double v) {
         // choosing a form also resets C~ to that form's default (the explicit damping of the displacement form
         // diverges at 0.55 on small grids)
         case DR_FORM:      if (v != 0.0 && v != 1.0) break; H->form = (int)v; H->cfl = H->form ? 0.50 : 0.55; H->have_fields = false; return DR_OK;
+        case DR_PALETTE:   if (v != 0.0 && v != 1.0) break; H->use_pal = (int)v; return DR_OK;
         case DR_ZCHUNK:    if (!(v >= 0.0) || v > 8192.0) break; H->fused_lz = v >= 1.0 ? (int)v : choose_lz(H->L); return DR_OK;
         default: break;
     }
@@ -269,6 +315,7 @@ static dr_status prepare(dr_handle* H, int lc, double eps0) {
     if (H->void_applied != H->void_rel) {
         k_void_clamp<<<(unsigned)((L.count + 255) / 256), 256, 0, H->st>>>(H->L, H->K0, H->G0, H->K, H->G, H->void_rel * H->hmax);
         CKL("k_void_clamp");
+        if (H->has_pal) { k_pal_values<<<1, 256, 0, H->st>>>(H->palK, H->palG, H->pal, H->void_rel * H->hmax); CKL("k_pal_values"); }
         H->void_applied = H->void_rel;
     }
     DrPT P = make_pt(H, lc, eps0);
@@ -311,9 +358,12 @@ static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
         T.m[4] = H->tm_K; T.m[5] = H->tm_state[c][F_SXX]; T.m[6] = H->tm_state[c][F_SYY]; T.m[7] = H->tm_state[c][F_SZZ];
         T.m[8] = H->tm_state[c][F_TXY]; T.m[9] = H->tm_state[c][F_TXZ]; T.m[10] = H->tm_state[c][F_TYZ];
         T.l2_hint = 0x1000000000000000ull;      // L2 evict_normal (evict_first measured 20 % slower, evict_last no gain)
-        const size_t smem_t = DrTmaCfg2<FUSED_TX, FUSED_TY>::SMEM2;
+        const bool palp = H->has_pal && H->use_pal;          // phase-id path: same values through a 256-entry table
+        T.mid = H->tm_ids; T.pal = H->pal;
+        const size_t smem_t = palp ? DrTmaCfg2<FUSED_TX, FUSED_TY, 1>::SMEM2 : DrTmaCfg2<FUSED_TX, FUSED_TY, 0>::SMEM2;
         DrFields Bo = fields_of(H, c ^ 1);
-#define DR_TMA(G_, R_, F_) k_pt_tma<G_, R_, F_, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits)
+#define DR_TMA(G_, R_, F_) do { if (palp) k_pt_tma<G_, R_, F_, 1, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); \
+                                else      k_pt_tma<G_, R_, F_, 0, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); } while (0)
         const int sel = (H->gavg ? 4 : 0) | (with_res ? 2 : 0) | (H->form ? 1 : 0);
         switch (sel) {
             case 0: DR_TMA(0, 0, 0); break; case 1: DR_TMA(0, 0, 1); break; case 2: DR_TMA(0, 1, 0); break; case 3: DR_TMA(0, 1, 1); break;
@@ -629,6 +679,8 @@ extern "C" dr_status dr_contribution_tensor(const double C_eff[36], const double
     for (int a = 0; a < 36; ++a) H_out[a] = (Se[a] - S1[a]) / phi;
     return DR_OK;
 }
+
+extern "C" int dr_uses_palette(dr_handle* H) { return (H && H->has_pal && H->use_pal && H->kernel == 0) ? 1 : 0; }
 
 extern "C" long long dr_launch_count(dr_handle* H) { return H ? H->launches : 0; }
 

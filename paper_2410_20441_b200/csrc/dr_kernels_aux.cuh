@@ -199,3 +199,79 @@ __global__ void k_export(DrLayout L, const double* __restrict__ src, double* __r
     if (i >= ex || j >= ey || k >= ez) return;
     dst[(size_t)i + (size_t)ex * ((size_t)j + (size_t)ey * k)] = src[L.origin + i + L.sy * j + L.sz * k];
 }
+
+// ------------------------------------------------------------------------------------------------------
+// Palette of the distinct (K,G) pairs (at most 256): phase-id path of the fused kernel.
+// keys: kK[256], kG[256] bit patterns, DR_PAL_EMPTY where unused (all-ones is a NaN pattern: moduli are validated
+// finite, so it never collides).  Open addressing, linear probing from a hash of both patterns.
+#define DR_PAL_EMPTY 0xffffffffffffffffull
+
+__device__ __forceinline__ unsigned dr_pal_hash(unsigned long long kb, unsigned long long gb) {
+    unsigned long long x = kb * 0x9E3779B97F4A7C15ull ^ (gb + 0x7F4A7C15ull) * 0xC2B2AE3D27D4EB4Full;
+    return (unsigned)(x >> 56);
+}
+
+// insert (or find) the pair; returns the slot, or -1 when all 256 slots hold other pairs
+__device__ __forceinline__ int dr_pal_insert(unsigned long long* kK, unsigned long long* kG, unsigned long long kb, unsigned long long gb) {
+    const unsigned h = dr_pal_hash(kb, gb);
+    for (int p = 0; p < 256; ++p) {
+        const int slot = (h + p) & 255;
+        unsigned long long ok = kK[slot];
+        if (ok == DR_PAL_EMPTY) ok = atomicCAS(kK + slot, DR_PAL_EMPTY, kb);
+        if (ok == DR_PAL_EMPTY || ok == kb) {
+            unsigned long long og = kG[slot];
+            if (og == DR_PAL_EMPTY) og = atomicCAS(kG + slot, DR_PAL_EMPTY, gb);
+            if (og == DR_PAL_EMPTY || og == gb) return slot;
+        }
+    }
+    return -1;
+}
+
+// lookup only (table complete): slot of the pair, -1 if absent
+__device__ __forceinline__ int dr_pal_find(const unsigned long long* kK, const unsigned long long* kG, unsigned long long kb, unsigned long long gb) {
+    const unsigned h = dr_pal_hash(kb, gb);
+    for (int p = 0; p < 256; ++p) {
+        const int slot = (h + p) & 255;
+        if (kK[slot] == kb && kG[slot] == gb) return slot;
+        if (kK[slot] == DR_PAL_EMPTY) return -1;
+    }
+    return -1;
+}
+
+// pass 1: every cell inserts its pair (consecutive equal cells are skipped); flags[0] |= 2 when the table overflows
+__global__ void k_pal_build(long long N, const double* __restrict__ Ksrc, const double* __restrict__ Gsrc,
+                            unsigned long long* kK, unsigned long long* kG, unsigned int* flags) {
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= N || (*((volatile unsigned int*)flags) & 2u)) return;
+    const unsigned long long kb = (unsigned long long)__double_as_longlong(Ksrc[q]), gb = (unsigned long long)__double_as_longlong(Gsrc[q]);
+    if (q > 0 && (threadIdx.x & 31) != 0) {          // same pair as the previous cell of the warp: that lane inserts it
+        if ((unsigned long long)__double_as_longlong(Ksrc[q - 1]) == kb && (unsigned long long)__double_as_longlong(Gsrc[q - 1]) == gb) return;
+    }
+    if (dr_pal_insert(kK, kG, kb, gb) < 0) atomicOr(flags, 2u);
+}
+
+// pass 2: phase id of every cell of the padded box (replicate halo like the moduli); flags[0] |= 4 on a miss
+__global__ void k_pal_assign(DrLayout L, const double* __restrict__ Ksrc, const double* __restrict__ Gsrc,
+                             const unsigned long long* __restrict__ kK, const unsigned long long* __restrict__ kG,
+                             unsigned char* __restrict__ ids, unsigned int* flags) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x - 1;      // -1 .. nx
+    int j = blockIdx.y * blockDim.y + threadIdx.y - 1;      // -1 .. ny
+    int k = blockIdx.z - 1;                                  // -1 .. nz
+    if (i > L.nx || j > L.ny) return;
+    int ci = min(max(i, 0), L.nx - 1), cj = min(max(j, 0), L.ny - 1), ck = min(max(k, 0), L.nz - 1);
+    size_t s = (size_t)ci + (size_t)L.nx * ((size_t)cj + (size_t)L.ny * ck);
+    const int slot = dr_pal_find(kK, kG, (unsigned long long)__double_as_longlong(Ksrc[s]), (unsigned long long)__double_as_longlong(Gsrc[s]));
+    if (slot < 0) { atomicOr(flags, 4u); return; }
+    ids[L.origin + i + L.sy * j + L.sz * k] = (unsigned char)slot;
+}
+
+// palette values K[256], G[256] from the keys, with the optional void clamp (same rule as k_void_clamp)
+__global__ void k_pal_values(const unsigned long long* __restrict__ kK, const unsigned long long* __restrict__ kG, double* pal, double thr) {
+    const int e = threadIdx.x;
+    double Kv = 0.0, Gv = 0.0;
+    if (kK[e] != DR_PAL_EMPTY && kG[e] != DR_PAL_EMPTY) {
+        Kv = __longlong_as_double((long long)kK[e]); Gv = __longlong_as_double((long long)kG[e]);
+        if (thr > 0.0 && Kv + 4.0 * Gv / 3.0 <= thr) { Kv = 0.0; Gv = 0.0; }
+    }
+    pal[e] = Kv; pal[256 + e] = Gv;
+}

@@ -19,23 +19,30 @@
 
 #define DR_TMA_SA 4
 #define DR_TMA_SB 3
-#define DR_TMA_NA 4      // fields per ring-A slot
-#define DR_TMA_NB 7      // fields per ring-B slot
+#define DR_TMA_NA 4      // fields per ring-A slot (3 with the palette: no G plane)
+#define DR_TMA_NB 7      // fields per ring-B slot (6 with the palette: no K plane)
+#define DR_ID_ROW 64     // bytes per row of the phase-id box (32 ids + up to 14 bytes of alignment slack, 16-byte multiple)
 
-// tensor maps of one launch: 0..3 = vx vy vz G, 4..10 = K sxx syy szz txy txz tyz (old state + moduli)
-struct DrTmaps { CUtensorMap m[DR_TMA_NA + DR_TMA_NB]; unsigned long long l2_hint; };
+// PAL = 1 (palette path): images with at most 256 distinct (K,G) pairs -- every segmented rock image -- keep a uint8
+// phase id per cell; the kernel stages the id box instead of the two fp64 modulus boxes and looks K, G up in a
+// 256-entry table in shared memory.  Same arithmetic on the same values, 14 B less HBM traffic per voxel-iteration.
+// tensor maps of one launch: 0..3 = vx vy vz G, 4..10 = K sxx syy szz txy txz tyz (old state + moduli); mid = phase ids
+struct DrTmaps { CUtensorMap m[DR_TMA_NA + DR_TMA_NB]; CUtensorMap mid; const double* pal; unsigned long long l2_hint; };
 
-template <int TX, int TY>
+template <int TX, int TY, int PAL = 0>
 struct DrTmaCfg {
     static constexpr int PL = TX * TY;                               // doubles per dense plane
+    static constexpr int NA = PAL ? DR_TMA_NA - 1 : DR_TMA_NA;       // planes per ring-A slot
+    static constexpr int NB = PAL ? DR_TMA_NB - 1 : DR_TMA_NB;       // planes per ring-B slot
+    static constexpr int BK = PAL ? 0 : 1;                           // first state plane of a ring-B slot (K sits before it)
     static constexpr int FRONT = 128;                                // pad (doubles) before the first plane
     static constexpr int RING_A = FRONT;                             // [SA][NA][PL]
-    static constexpr int RING_B = RING_A + DR_TMA_SA * DR_TMA_NA * PL;   // [SB][NB][PL]
-    static constexpr int XCH = RING_B + DR_TMA_SB * DR_TMA_NB * PL;  // 5 single + 4 double planes
+    static constexpr int RING_B = RING_A + DR_TMA_SA * NA * PL;      // [SB][NB][PL]
+    static constexpr int XCH = RING_B + DR_TMA_SB * NB * PL;         // exchange planes
     static constexpr int END = XCH + 13 * PL;
     static constexpr size_t SMEM = (size_t)(END + 64) * sizeof(double);
-    static constexpr unsigned BYTES_A = DR_TMA_NA * PL * sizeof(double);
-    static constexpr unsigned BYTES_B = DR_TMA_NB * PL * sizeof(double);
+    static constexpr unsigned BYTES_A = NA * PL * sizeof(double);
+    static constexpr unsigned BYTES_B = NB * PL * sizeof(double);
 };
 
 __device__ __forceinline__ unsigned dr_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -66,24 +73,25 @@ __device__ __forceinline__ void dr_tma_load_3d(void* dst, const CUtensorMap* map
 // one batch: ring-A fields of layer m (z = m+1 in the padded box) and, if with_b, the ring-B set m:
 //   FORM 0: K, sigma_xx, sigma_yy, sigma_zz, tau_xy of layer m-1 and tau_xz, tau_yz of face m
 //   FORM 1: K, w_x, w_y, w_z of layer m-1 (w lives in the sigma_aa slots of the state buffer)
-template <int FORM, int TX, int TY>
+template <int FORM, int PAL, int TX, int TY>
 __device__ __forceinline__ void dr_tma_issue_batch(const DrTmaps& T, unsigned long long* bar, double* da, double* db,
-                                                   int x0, int y0, int m, bool with_b) {
+                                                   unsigned char* idd, int x0, int xa, int y0, int m, bool with_b) {
     constexpr int PL = TX * TY;
-    constexpr unsigned BA = DR_TMA_NA * PL * sizeof(double);
-    constexpr unsigned BB = (FORM ? 4 : DR_TMA_NB) * PL * sizeof(double);
+    constexpr unsigned BA = 3 * PL * sizeof(double) + (PAL ? DR_ID_ROW * TY : PL * sizeof(double));
+    constexpr unsigned BB = ((FORM ? 3 : 6) + (PAL ? 0 : 1)) * PL * sizeof(double);
+    constexpr int BK = PAL ? 0 : 1;
     dr_mbar_expect_tx(bar, with_b ? BA + BB : BA);
 #pragma unroll
-    for (int f = 0; f < DR_TMA_NA; ++f) dr_tma_load_3d(da + f * PL, &T.m[f], bar, x0, y0, m + 1, T.l2_hint);
+    for (int f = 0; f < 3; ++f) dr_tma_load_3d(da + f * PL, &T.m[f], bar, x0, y0, m + 1, T.l2_hint);
+    if (PAL) dr_tma_load_3d(idd, &T.mid, bar, xa, y0, m + 1, T.l2_hint);
+    else     dr_tma_load_3d(da + 3 * PL, &T.m[3], bar, x0, y0, m + 1, T.l2_hint);
     if (with_b) {
-        if (FORM) {
+        if (!PAL) dr_tma_load_3d(db, &T.m[4], bar, x0, y0, m, T.l2_hint);                   // K of layer m-1
 #pragma unroll
-            for (int f = 0; f < 4; ++f) dr_tma_load_3d(db + f * PL, &T.m[DR_TMA_NA + f], bar, x0, y0, m, T.l2_hint);
-        } else {
-#pragma unroll
-            for (int f = 0; f < 5; ++f) dr_tma_load_3d(db + f * PL, &T.m[DR_TMA_NA + f], bar, x0, y0, m, T.l2_hint);
-            dr_tma_load_3d(db + 5 * PL, &T.m[DR_TMA_NA + 5], bar, x0, y0, m + 1, T.l2_hint);
-            dr_tma_load_3d(db + 6 * PL, &T.m[DR_TMA_NA + 6], bar, x0, y0, m + 1, T.l2_hint);
+        for (int f = 0; f < (FORM ? 3 : 4); ++f) dr_tma_load_3d(db + (BK + f) * PL, &T.m[5 + f], bar, x0, y0, m, T.l2_hint);
+        if (!FORM) {
+            dr_tma_load_3d(db + (BK + 4) * PL, &T.m[9], bar, x0, y0, m + 1, T.l2_hint);
+            dr_tma_load_3d(db + (BK + 5) * PL, &T.m[10], bar, x0, y0, m + 1, T.l2_hint);
         }
     }
 }
@@ -95,37 +103,45 @@ struct DrCarry { double txz, tyz, gxz, gyz, szz, hc, txz_r, tyz_u, gxz_r, gyz_u;
 // exchange planes (doubles, relative to XCH), double-buffered by step parity: [2][9][PL]
 enum { X_SXX = 0, X_SYY, X_TXY, X_HC, X_GXY, X_TXZ, X_TYZ, X_GXZ, X_GYZ, X_COUNT };
 
-template <int TX, int TY>
-struct DrTmaCfg2 : DrTmaCfg<TX, TY> {
-    using B = DrTmaCfg<TX, TY>;
+template <int TX, int TY, int PAL = 0>
+struct DrTmaCfg2 : DrTmaCfg<TX, TY, PAL> {
+    using B = DrTmaCfg<TX, TY, PAL>;
     static constexpr int END2 = B::XCH + 2 * X_COUNT * B::PL;
     static constexpr size_t SMEM2 = (size_t)(END2 + 64) * sizeof(double);
 };
 
-template <int GAVG, int RES, int FORM, int TX, int TY, bool BND, int PAR>
+template <int GAVG, int RES, int FORM, int PAL, int TX, int TY, bool BND, int PAR>
 __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, const DrTmaps& T, const DrFusedPtrs& g,
-                                            double* sm, unsigned long long* bars, const int s, const int t, const int k,
+                                            double* sm, unsigned char* idr, const double* pal, const int sid, const int xa,
+                                            unsigned long long* bars, const int s, const int t, const int k,
                                             const int kb, const int ke, const bool store, const int i, const int j,
                                             const int x0, const int y0, const bool producer, const bool midrow, const bool inner,
                                             const DrCarry& fc, DrCarry& fn, double& rmax, bool& rnan) {
-    using Cfg = DrTmaCfg2<TX, TY>;
-    constexpr int PL = Cfg::PL;
+    using Cfg = DrTmaCfg2<TX, TY, PAL>;
+    constexpr int PL = Cfg::PL, BK = Cfg::BK;
     const int nx = L.nx, ny = L.ny, nz = L.nz;
     const long long sz = L.sz;
     const double h = P.h, ih = P.inv_h, th = P.theta, ri = P.rinv, c2t = P.c2t;
-    const double* Ac = sm + Cfg::RING_A + (t & 3) * (DR_TMA_NA * PL) + s;          // layer k
-    const double* An = sm + Cfg::RING_A + ((t + 1) & 3) * (DR_TMA_NA * PL) + s;    // layer k+1
-    const double* Bs = sm + Cfg::RING_B + (t % 3) * (DR_TMA_NB * PL) + s;          // set k+1
+    const double* Ac = sm + Cfg::RING_A + (t & 3) * (Cfg::NA * PL) + s;            // layer k
+    const double* An = sm + Cfg::RING_A + ((t + 1) & 3) * (Cfg::NA * PL) + s;      // layer k+1
+    const double* Bs = sm + Cfg::RING_B + (t % 3) * (Cfg::NB * PL) + s;            // set k+1
+    const unsigned char* Ic = idr + (t & 3) * (DR_ID_ROW * TY) + sid;               // phase ids of layer k   (PAL)
+    const unsigned char* In = idr + ((t + 1) & 3) * (DR_ID_ROW * TY) + sid;         // phase ids of layer k+1 (PAL)
+    // moduli of the own cell and of its -x / -y neighbours: from the fp64 planes, or through the palette (pal[id] = K,
+    // pal[256 + id] = G)
+    auto Gof = [&](const double* A, const unsigned char* I, int dx, int dy) -> double {
+        return PAL ? pal[256 + I[dy * DR_ID_ROW + dx]] : A[3 * PL + dy * TX + dx];
+    };
     double* X = sm + Cfg::XCH + PAR * (X_COUNT * PL) + s;                           // this step's exchange planes
 
     // batch t+1 (layer k+1, set k+1) has landed: it was waited for behind the barrier of the previous step
 
     // ================= stage A: new stresses =================
-    const double vxc = Ac[0 * PL], vyc = Ac[1 * PL], vzc = Ac[2 * PL], Gc = Ac[3 * PL];
-    const double vxn = An[0 * PL], vyn = An[1 * PL], vzn = An[2 * PL], Gn = An[3 * PL];
-    const double Kc = Bs[0 * PL];
+    const double vxc = Ac[0 * PL], vyc = Ac[1 * PL], vzc = Ac[2 * PL], Gc = Gof(Ac, Ic, 0, 0);
+    const double vxn = An[0 * PL], vyn = An[1 * PL], vzn = An[2 * PL], Gn = Gof(An, In, 0, 0);
+    const double Kc = PAL ? pal[Ic[0]] : Bs[0];
     // FORM 1: the old w must be read HERE: after the barrier below the ring-B slot is handed back to the TMA unit
-    const double wxo = FORM ? Bs[1 * PL] : 0.0, wyo = FORM ? Bs[2 * PL] : 0.0, wzo = FORM ? Bs[3 * PL] : 0.0;
+    const double wxo = FORM ? Bs[(BK + 0) * PL] : 0.0, wyo = FORM ? Bs[(BK + 1) * PL] : 0.0, wzo = FORM ? Bs[(BK + 2) * PL] : 0.0;
     const bool bk1 = (k + 1 == 0 || k + 1 == nz);
     const double dxx = (Ac[0 * PL + 1] - vxc) * ih;
     const double dyy = (Ac[1 * PL + TX] - vyc) * ih;
@@ -133,12 +149,12 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
     const double lam_div = fma(-(2.0 / 3.0), Gc, Kc) * (dxx + dyy + dzz);
     const double g2 = 2.0 * Gc;
     // FORM 0: relaxation toward Hooke's law (Eq. 12-13); FORM 1 (displacement form): Hooke's law itself
-    const double nsxx = FORM ? fma(g2, dxx, lam_div) : (Bs[1 * PL] + th * fma(g2, dxx, lam_div)) * ri;
-    const double nsyy = FORM ? fma(g2, dyy, lam_div) : (Bs[2 * PL] + th * fma(g2, dyy, lam_div)) * ri;
-    const double nszz = FORM ? fma(g2, dzz, lam_div) : (Bs[3 * PL] + th * fma(g2, dzz, lam_div)) * ri;
+    const double nsxx = FORM ? fma(g2, dxx, lam_div) : (Bs[(BK + 0) * PL] + th * fma(g2, dxx, lam_div)) * ri;
+    const double nsyy = FORM ? fma(g2, dyy, lam_div) : (Bs[(BK + 1) * PL] + th * fma(g2, dyy, lam_div)) * ri;
+    const double nszz = FORM ? fma(g2, dzz, lam_div) : (Bs[(BK + 2) * PL] + th * fma(g2, dzz, lam_div)) * ri;
     const double hc = fma(4.0 / 3.0, Gc, Kc);
-    const double gl = Ac[3 * PL - 1], gd = Ac[3 * PL - TX], gld = Ac[3 * PL - TX - 1];
-    const double gln = An[3 * PL - 1], gdn = An[3 * PL - TX];
+    const double gl = Gof(Ac, Ic, -1, 0), gd = Gof(Ac, Ic, 0, -1), gld = Gof(Ac, Ic, -1, -1);
+    const double gln = Gof(An, In, -1, 0), gdn = Gof(An, In, 0, -1);
     const double gxy = dr_edge_mean_fast<GAVG>(gld, gd, gl, Gc);
     const double gxz = dr_edge_mean_fast<GAVG>(gl, Gc, gln, Gn);
     const double gyz = dr_edge_mean_fast<GAVG>(gd, Gc, gdn, Gn);
@@ -170,9 +186,9 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
             + dr_dshear(vzn, vzn_d, j, ny, dr_u0(P, 2, x, j == 0 ? 0.0 : P.Ly, (k + 1) * h));
         zyz = false;
     }
-    const double ntxy = zxy ? 0.0 : (FORM ? gxy * (exy * ih) : (Bs[4 * PL] + th * gxy * (exy * ih)) * ri);
-    const double ntxz = zxz ? 0.0 : (FORM ? gxz * (exz * ih) : (Bs[5 * PL] + th * gxz * (exz * ih)) * ri);
-    const double ntyz = zyz ? 0.0 : (FORM ? gyz * (eyz * ih) : (Bs[6 * PL] + th * gyz * (eyz * ih)) * ri);
+    const double ntxy = zxy ? 0.0 : (FORM ? gxy * (exy * ih) : (Bs[(BK + 3) * PL] + th * gxy * (exy * ih)) * ri);
+    const double ntxz = zxz ? 0.0 : (FORM ? gxz * (exz * ih) : (Bs[(BK + 4) * PL] + th * gxz * (exz * ih)) * ri);
+    const double ntyz = zyz ? 0.0 : (FORM ? gyz * (eyz * ih) : (Bs[(BK + 5) * PL] + th * gyz * (eyz * ih)) * ri);
 
     X[X_SXX * PL] = nsxx; X[X_SYY * PL] = nsyy; X[X_TXY * PL] = ntxy; X[X_HC * PL] = hc; X[X_GXY * PL] = gxy;
     X[X_TXZ * PL] = ntxz; X[X_TYZ * PL] = ntyz; X[X_GXZ * PL] = gxz; X[X_GYZ * PL] = gyz;
@@ -183,9 +199,9 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
     if (producer && k + 4 <= ke) {
         const int b = t + 4, m = k + 4;
         unsigned long long* bar = bars + (b & 3);
-        double* da = sm + Cfg::RING_A + (b & 3) * (DR_TMA_NA * PL);
-        double* db = sm + Cfg::RING_B + ((b - 1) % 3) * (DR_TMA_NB * PL);
-        dr_tma_issue_batch<FORM, TX, TY>(T, bar, da, db, x0, y0, m, true);
+        double* da = sm + Cfg::RING_A + (b & 3) * (Cfg::NA * PL);
+        double* db = sm + Cfg::RING_B + ((b - 1) % 3) * (Cfg::NB * PL);
+        dr_tma_issue_batch<FORM, PAL, TX, TY>(T, bar, da, db, idr + (b & 3) * (DR_ID_ROW * TY), x0, xa, y0, m, true);
     }
     // ---- wait HERE for the batch of the next step (issued two steps ago), not at the top of the next step: stage B
     // below and stage A of the next step then form one straight-line region that the scheduler can interleave
@@ -260,9 +276,10 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
     }
 }
 
-template <int GAVG, int RES, int FORM, int TX, int TY, bool BND>
+template <int GAVG, int RES, int FORM, int PAL, int TX, int TY, bool BND>
 __device__ __forceinline__ void dr_tma_march(const DrLayout& L, const DrPT& P, const DrTmaps& T, const DrFusedPtrs& g,
-                                             double* sm, unsigned long long* bars, const int s, const int kb, const int ke,
+                                             double* sm, unsigned char* idr, const double* pal, const int sid, const int xa,
+                                             unsigned long long* bars, const int s, const int kb, const int ke,
                                              const int i, const int j, const int x0, const int y0,
                                              const bool producer, const bool midrow, const bool inner, double& rmax, bool& rnan) {
     DrCarry fa, fb;
@@ -270,18 +287,21 @@ __device__ __forceinline__ void dr_tma_march(const DrLayout& L, const DrPT& P, c
     fb = fa;
     int k = kb - 1;
     for (int t = 0; k < ke; t += 2, k += 2) {
-        dr_tma_step<GAVG, RES, FORM, TX, TY, BND, 0>(L, P, T, g, sm, bars, s, t, k, kb, ke, k >= kb, i, j, x0, y0, producer, midrow, inner, fa, fb, rmax, rnan);
+        dr_tma_step<GAVG, RES, FORM, PAL, TX, TY, BND, 0>(L, P, T, g, sm, idr, pal, sid, xa, bars, s, t, k, kb, ke, k >= kb, i, j, x0, y0, producer, midrow, inner, fa, fb, rmax, rnan);
         if (k + 1 < ke)
-            dr_tma_step<GAVG, RES, FORM, TX, TY, BND, 1>(L, P, T, g, sm, bars, s, t + 1, k + 1, kb, ke, true, i, j, x0, y0, producer, midrow, inner, fb, fa, rmax, rnan);
+            dr_tma_step<GAVG, RES, FORM, PAL, TX, TY, BND, 1>(L, P, T, g, sm, idr, pal, sid, xa, bars, s, t + 1, k + 1, kb, ke, true, i, j, x0, y0, producer, midrow, inner, fb, fa, rmax, rnan);
     }
 }
 
-template <int GAVG, int RES, int FORM, int TX, int TY>
+template <int GAVG, int RES, int FORM, int PAL, int TX, int TY>
 __global__ void __launch_bounds__(TX * TY, 1)
 k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int lz, unsigned long long* res_bits) {
     extern __shared__ __align__(1024) double sm[];
     __shared__ __align__(8) unsigned long long bars[4];
-    using Cfg = DrTmaCfg2<TX, TY>;
+    __shared__ __align__(128) unsigned char idr_raw[PAL ? 128 + 4 * DR_ID_ROW * TY + 128 : 16];   // id ring + slack for -1 row reads
+    __shared__ double pal[PAL ? 512 : 1];                                                          // K[256], G[256]
+    unsigned char* idr = idr_raw + (PAL ? 128 : 0);
+    using Cfg = DrTmaCfg2<TX, TY, PAL>;
     constexpr int PL = Cfg::PL;
     const int nx = L.nx, ny = L.ny, nz = L.nz;
     const int tx = threadIdx.x, ty = threadIdx.y;
@@ -290,7 +310,10 @@ k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int 
     const int kb = blockIdx.z * lz;                          // first output layer of this chunk
     const int ke = min(kb + lz, nz + 1);                     // one past the last output layer (layer nz = top faces)
     const int x0 = DR_OX + i0 - 1, y0 = j0;                  // box origin in padded-field coordinates (z = layer + 1)
+    const int xa = x0 & ~15;                                 // id box origin: 16-byte aligned (TMA), x0 - xa in {0,2,..,14}
+    const int sid = ty * DR_ID_ROW + (x0 - xa) + tx;         // own id inside an id slot
     const int s = ty * TX + tx;
+    if (PAL) for (int e = s; e < 512; e += TX * TY) pal[e] = T.pal[e];
     const bool producer = (tx == 0 && ty == 0);
     const bool midrow = ty >= 1 && ty <= TY - 2;
     const bool inner = tx >= 1 && tx <= TX - 2 && i <= nx && j <= ny;
@@ -306,9 +329,9 @@ k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int 
             const int m = kb - 1 + b;
             if (m <= ke) {
                 unsigned long long* bar = bars + b;
-                double* da = sm + Cfg::RING_A + b * (DR_TMA_NA * PL);
-                double* db = sm + Cfg::RING_B + (b >= 1 ? b - 1 : 0) * (DR_TMA_NB * PL);
-                dr_tma_issue_batch<FORM, TX, TY>(T, bar, da, db, x0, y0, m, b >= 1);
+                double* da = sm + Cfg::RING_A + b * (Cfg::NA * PL);
+                double* db = sm + Cfg::RING_B + (b >= 1 ? b - 1 : 0) * (Cfg::NB * PL);
+                dr_tma_issue_batch<FORM, PAL, TX, TY>(T, bar, da, db, idr + b * (DR_ID_ROW * TY), x0, xa, y0, m, b >= 1);
             }
         }
     }
@@ -324,8 +347,8 @@ k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int 
     double rmax = 0.0;
     bool rnan = false;
     const bool interior = i0 >= 2 && i0 + TX - 2 <= nx - 1 && j0 >= 2 && j0 + TY - 2 <= ny - 1;
-    if (interior) dr_tma_march<GAVG, RES, FORM, TX, TY, false>(L, P, T, g, sm, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
-    else          dr_tma_march<GAVG, RES, FORM, TX, TY, true>(L, P, T, g, sm, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
+    if (interior) dr_tma_march<GAVG, RES, FORM, PAL, TX, TY, false>(L, P, T, g, sm, idr, pal, sid, xa, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
+    else          dr_tma_march<GAVG, RES, FORM, PAL, TX, TY, true>(L, P, T, g, sm, idr, pal, sid, xa, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
 
     if (RES) {
         __shared__ unsigned long long smr[32];

@@ -42,7 +42,7 @@ def field_errors(o, s, K, G, eps0, h=1.0):
 
 
 def run_pair(oracle_mod, gpu, K, G, lc, eps0, niter, h=1.0, **params):
-    o = oracle_mod.Oracle(K, G, h=h, **{k: v for k, v in params.items() if k not in ("kernel", "zchunk")})
+    o = oracle_mod.Oracle(K, G, h=h, **{k: v for k, v in params.items() if k not in ("kernel", "zchunk", "palette")})
     s = gpu.Solver(to_dev(K), to_dev(G), h=h, **params)
     o.step(lc, eps0, niter)
     s.step(lc, eps0, niter)
@@ -372,3 +372,40 @@ def test_fuzz_random_shapes_and_parameters(oracle_mod, gpu, seed):
     errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, eps0, niter, h=h, **params)
     assert max(errs) <= FIELD_TOL, (shape, params, lc, niter, errs)
     assert np.isfinite(rs) and abs(ro - rs) <= 1e-9 * max(ro, 1e-300), (shape, params, ro, rs)
+
+
+def _quantised(shape, levels, seed):
+    """image with `levels` distinct (K,G) pairs: exercises the phase-id (palette) path of the fused kernel"""
+    rng = np.random.default_rng(seed)
+    sh = tuple(shape)[::-1]
+    ph = rng.integers(0, levels, size=sh)
+    Kt = rng.uniform(1.0, 70.0, size=levels); Gt = rng.uniform(0.5, 45.0, size=levels)
+    if levels > 3:
+        Kt[1] = Gt[1] = 0.0          # a void phase
+        Gt[2] = 0.0                  # a fluid phase
+    return np.ascontiguousarray(Kt[ph]), np.ascontiguousarray(Gt[ph])
+
+
+@pytest.mark.parametrize("levels", [1, 2, 7, 256, 300])
+@pytest.mark.parametrize("palette", [1, 0])
+def test_palette_path_matches_oracle(oracle_mod, gpu, levels, palette):
+    """<= 256 distinct pairs -> uint8 phase ids + table; 300 -> falls back to the fp64 fields.  Same values either way."""
+    K, G = _quantised((45, 33, 21), levels, seed=levels)
+    for lc, extra in ((2, {}), (5, dict(bc_mode=1, gavg=1)), (3, dict(form=1)), (0, dict(void_rel=0.2))):
+        errs, ro, rs, _, _ = run_pair(oracle_mod, gpu, K, G, lc, 1e-4, 14, h=0.8, palette=palette, **extra)
+        assert max(errs) <= FIELD_TOL, (levels, palette, lc, errs)
+        assert abs(ro - rs) <= 1e-9 * ro + 1e-13          # a one-phase image has residual ~1e-16
+    s = gpu.Solver(to_dev(K), to_dev(G), palette=palette)
+    assert s.uses_palette() == (palette == 1 and levels <= 256)
+
+
+def test_palette_path_is_bitwise_the_fp64_path(gpu):
+    import torch
+    K, G, _ = inputs.config3_random_spheres(n=96, npores=40)
+    res = []
+    for palette in (1, 0):
+        s = gpu.Solver(to_dev(K), to_dev(G), palette=palette)
+        s.step(4, 1e-4, 25)
+        res.append([s.get_field(f).clone() for f in range(9)] + [torch.tensor(s.info()[1])])
+    for a, b in zip(*res):
+        assert torch.equal(a, b)
