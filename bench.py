@@ -180,6 +180,7 @@ def main():
     ap.add_argument("--ncheck", type=int, default=100)
     ap.add_argument("--kernel", type=int, default=0, help="0 fused with TMA staging (default), 1 split baseline, 2 fused with LDG prefetch")
     ap.add_argument("--form", type=int, default=0, help="0 stress-relaxation form of the paper (default, 160 B/voxel), 1 displacement form (112 B/voxel)")
+    ap.add_argument("--palette", type=int, default=1, help="1 (default): uint8 phase ids + table when the image has <= 256 distinct (K,G); 0: fp64 modulus fields")
     ap.add_argument("--cpu-sample-n", type=int, default=191)
     ap.add_argument("--cpu-iters", type=int, default=100)
     ap.add_argument("--cpu-iters-per-step", type=int, default=5)
@@ -215,7 +216,7 @@ def main():
     lc = shard.load_case_of_rank(rank, world, args.lc)
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
-        s = binding.Solver(Kd, Gd, stream=stream, ncheck=args.ncheck, kernel=args.kernel, form=args.form)
+        s = binding.Solver(Kd, Gd, stream=stream, ncheck=args.ncheck, kernel=args.kernel, form=args.form, palette=args.palette)
 
         def barrier():
             torch.cuda.synchronize(dev)
@@ -236,6 +237,7 @@ def main():
         e1.record(stream)
         barrier()
         launches = s.launch_count() - l0
+        pal_active = s.uses_palette()
         ms = e0.elapsed_time(e1)
         # ---- dominant kernel alone (k_pt_fused back to back, no residual): average launch duration
         s.iterate(lc, args.eps0, 5)
@@ -272,7 +274,7 @@ def main():
             del stage, Kh, Gh
             # the solver's workspace was reused by the e2e call: rebuild the handle state
             s.close()
-            s = binding.Solver(Kd, Gd, stream=stream, workspace=s.workspace, ncheck=args.ncheck, kernel=args.kernel, form=args.form)
+            s = binding.Solver(Kd, Gd, stream=stream, workspace=s.workspace, ncheck=args.ncheck, kernel=args.kernel, form=args.form, palette=args.palette)
         if dist is not None:
             dist.barrier()
             dist.destroy_process_group()
@@ -300,7 +302,7 @@ def main():
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s: %s" % (args.workload, WORKLOADS[args.workload]["desc"]), "grid": [n, n, n],
-                   "load_case": lc, "ncheck": args.ncheck, "form": "stress-relaxation (paper, 160 B/voxel-iteration)" if args.form == 0 else "displacement (112 B/voxel-iteration)", "kernel": {0: "fused+TMA", 1: "split", 2: "fused+LDG"}[args.kernel],
+                   "load_case": lc, "ncheck": args.ncheck, "form": "stress-relaxation (paper, 160 B/voxel-iteration)" if args.form == 0 else "displacement (112 B/voxel-iteration)", "kernel": {0: "fused+TMA", 1: "split", 2: "fused+LDG"}[args.kernel], "moduli": "uint8 phase ids + 256-entry table" if pal_active else "fp64 K, G fields",
                    "parallelism": "load cases sharded over %d GPU(s), no collective" % world,
                    "l2": "inputs (%.1f GB per iteration) larger than L2; no flush needed" % (BYTES_PER_VOXEL_ITER * N / 1e9)},
         "T_eff_GBs": teff, "T_eff_frac_of_measured_peak": teff / peak, "T_eff_frac_of_8000_nominal": teff / 8000.0,

@@ -32,12 +32,11 @@ struct dr_handle {
     double* avg_dev;            // 6
     unsigned long long* res_bits;
     unsigned long long* hmax_bits;
-    unsigned char* ids;         // uint8 phase id per cell on the padded box (palette path)
+    unsigned char* ids;         // uint8 phase ids, tile-blocked (palette path)
     unsigned long long *palK, *palG;   // palette keys (bit patterns), 256 each
     double* pal;                // palette values K[256], G[256] after the void clamp
     bool has_pal;               // the image has at most 256 distinct (K,G) pairs
     int use_pal;                // DR_PALETTE
-    CUtensorMap tm_ids;
     unsigned int* flags;
     // host
     double* pinned;             // 8 doubles, page-locked
@@ -90,7 +89,10 @@ static bool sizes_ok(int nx, int ny, int nz) {
 static size_t field_bytes(const DrLayout& L) { return align_up((size_t)L.count * sizeof(double), 256); }
 static const int N_BIG = 2 * F_COUNT + 4;        // 18 state fields + K0, G0, K, G
 static const size_t SMALL_BYTES = align_up((size_t)DR_AVG_BLOCKS * 6 * sizeof(double), 256) + 1024 + 3 * 4096;   // + palette keys and values
-static size_t ids_bytes(const DrLayout& L) { return align_up((size_t)L.count, 256); }
+static int tiles_x(const DrLayout& L) { return (L.nx + 1 + FUSED_TX - 3) / (FUSED_TX - 2); }
+static int tiles_y(const DrLayout& L) { return (L.ny + 1 + FUSED_TY - 3) / (FUSED_TY - 2); }
+// tile-blocked phase ids: one FUSED_TX*FUSED_TY byte block per (tile, layer), layers -1 .. nz+1
+static size_t ids_bytes(const DrLayout& L) { return align_up((size_t)tiles_x(L) * tiles_y(L) * (L.nz + 3) * (FUSED_TX * FUSED_TY), 256); }
 
 extern "C" size_t dr_workspace_bytes(int nx, int ny, int nz) {
     if (!sizes_ok(nx, ny, nz)) return 0;
@@ -137,18 +139,6 @@ static bool make_tmap(dr_handle* H, dr_encode_fn enc, CUtensorMap* out, double* 
     return true;
 }
 
-static bool make_ids_tmap(dr_handle* H, dr_encode_fn enc) {
-    const DrLayout& L = H->L;
-    cuuint64_t dims[3] = {(cuuint64_t)L.PX, (cuuint64_t)L.PY, (cuuint64_t)L.PZ};
-    cuuint64_t strides[2] = {(cuuint64_t)L.PX, (cuuint64_t)L.PX * L.PY};          // bytes; PX is a multiple of 16
-    cuuint32_t box[3] = {DR_ID_ROW, FUSED_TY, 1};
-    cuuint32_t estr[3] = {1, 1, 1};
-    CUresult r = enc(&H->tm_ids, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, H->ids, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) { H->err = "cuTensorMapEncodeTiled(ids) failed (" + std::to_string((int)r) + ")"; return false; }
-    return true;
-}
-
 static bool make_all_tmaps(dr_handle* H) {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qr;
@@ -158,7 +148,7 @@ static bool make_all_tmaps(dr_handle* H) {
     }
     dr_encode_fn enc = (dr_encode_fn)fn;
     for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) if (!make_tmap(H, enc, &H->tm_state[b][f], H->buf[b][f])) return false;
-    return make_tmap(H, enc, &H->tm_K, H->K) && make_tmap(H, enc, &H->tm_G, H->G) && make_ids_tmap(H, enc);
+    return make_tmap(H, enc, &H->tm_K, H->K) && make_tmap(H, enc, &H->tm_G, H->G);
 }
 
 extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K, const double* G,
@@ -224,7 +214,7 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
             !cuda_ok(H, cudaStreamSynchronize(H->st), "cudaStreamSynchronize")) { st = DR_ERR_CUDA; break; }
         if (fl & 1u) { st = DR_ERR_ARG; break; }
         if (!(fl & 2u)) {
-            k_pal_assign<<<grd, blk, 0, H->st>>>(H->L, K, G, H->palK, H->palG, H->ids, H->flags);
+            k_pal_assign<<<dim3(tiles_x(H->L), tiles_y(H->L), nz + 3), dim3(FUSED_TX, FUSED_TY, 1), 0, H->st>>>(H->L, K, G, H->palK, H->palG, H->ids, H->flags);
             k_pal_values<<<1, 256, 0, H->st>>>(H->palK, H->palG, H->pal, 0.0);
             H->launches += 2;
             unsigned int fl2 = 0;
@@ -359,7 +349,7 @@ static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
         T.m[8] = H->tm_state[c][F_TXY]; T.m[9] = H->tm_state[c][F_TXZ]; T.m[10] = H->tm_state[c][F_TYZ];
         T.l2_hint = 0x1000000000000000ull;      // L2 evict_normal (evict_first measured 20 % slower, evict_last no gain)
         const bool palp = H->has_pal && H->use_pal;          // phase-id path: same values through a 256-entry table
-        T.mid = H->tm_ids; T.pal = H->pal;
+        T.ids = H->ids; T.pal = H->pal; T.gx = (int)grd.x; T.gy = (int)grd.y;
         const size_t smem_t = palp ? DrTmaCfg2<FUSED_TX, FUSED_TY, 1>::SMEM2 : DrTmaCfg2<FUSED_TX, FUSED_TY, 0>::SMEM2;
         DrFields Bo = fields_of(H, c ^ 1);
 #define DR_TMA(G_, R_, F_) do { if (palp) k_pt_tma<G_, R_, F_, 1, FUSED_TX, FUSED_TY><<<grd, blk, smem_t, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); \

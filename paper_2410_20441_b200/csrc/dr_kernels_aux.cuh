@@ -250,19 +250,22 @@ __global__ void k_pal_build(long long N, const double* __restrict__ Ksrc, const 
     if (dr_pal_insert(kK, kG, kb, gb) < 0) atomicOr(flags, 2u);
 }
 
-// pass 2: phase id of every cell of the padded box (replicate halo like the moduli); flags[0] |= 4 on a miss
+// pass 2: phase ids, TILE-BLOCKED for the fused kernel: block (bx, by, z) holds the TX*TY ids of the extended tile
+// (i0-1+tx, j0-1+ty) of layer z-1, i0 = bx (TX-2), j0 = by (TY-2), replicate-padded like the moduli; flags[0] |= 4 on a miss.
+// grid (gx, gy, nz+3), block (TX, TY).
 __global__ void k_pal_assign(DrLayout L, const double* __restrict__ Ksrc, const double* __restrict__ Gsrc,
                              const unsigned long long* __restrict__ kK, const unsigned long long* __restrict__ kG,
                              unsigned char* __restrict__ ids, unsigned int* flags) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x - 1;      // -1 .. nx
-    int j = blockIdx.y * blockDim.y + threadIdx.y - 1;      // -1 .. ny
-    int k = blockIdx.z - 1;                                  // -1 .. nz
-    if (i > L.nx || j > L.ny) return;
-    int ci = min(max(i, 0), L.nx - 1), cj = min(max(j, 0), L.ny - 1), ck = min(max(k, 0), L.nz - 1);
-    size_t s = (size_t)ci + (size_t)L.nx * ((size_t)cj + (size_t)L.ny * ck);
+    const int TX = blockDim.x, TY = blockDim.y;
+    const int i = blockIdx.x * (TX - 2) - 1 + threadIdx.x;
+    const int j = blockIdx.y * (TY - 2) - 1 + threadIdx.y;
+    const int k = (int)blockIdx.z - 1;
+    const int ci = min(max(i, 0), L.nx - 1), cj = min(max(j, 0), L.ny - 1), ck = min(max(k, 0), L.nz - 1);
+    const size_t s = (size_t)ci + (size_t)L.nx * ((size_t)cj + (size_t)L.ny * ck);
     const int slot = dr_pal_find(kK, kG, (unsigned long long)__double_as_longlong(Ksrc[s]), (unsigned long long)__double_as_longlong(Gsrc[s]));
     if (slot < 0) { atomicOr(flags, 4u); return; }
-    ids[L.origin + i + L.sy * j + L.sz * k] = (unsigned char)slot;
+    const size_t blk = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    ids[blk * (size_t)(TX * TY) + threadIdx.y * TX + threadIdx.x] = (unsigned char)slot;
 }
 
 // palette values K[256], G[256] from the keys, with the optional void clamp (same rule as k_void_clamp)

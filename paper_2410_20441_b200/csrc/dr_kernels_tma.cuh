@@ -21,13 +21,21 @@
 #define DR_TMA_SB 3
 #define DR_TMA_NA 4      // fields per ring-A slot (3 with the palette: no G plane)
 #define DR_TMA_NB 7      // fields per ring-B slot (6 with the palette: no K plane)
-#define DR_ID_ROW 64     // bytes per row of the phase-id box (32 ids + up to 14 bytes of alignment slack, 16-byte multiple)
 
 // PAL = 1 (palette path): images with at most 256 distinct (K,G) pairs -- every segmented rock image -- keep a uint8
-// phase id per cell; the kernel stages the id box instead of the two fp64 modulus boxes and looks K, G up in a
-// 256-entry table in shared memory.  Same arithmetic on the same values, 14 B less HBM traffic per voxel-iteration.
-// tensor maps of one launch: 0..3 = vx vy vz G, 4..10 = K sxx syy szz txy txz tyz (old state + moduli); mid = phase ids
-struct DrTmaps { CUtensorMap m[DR_TMA_NA + DR_TMA_NB]; CUtensorMap mid; const double* pal; unsigned long long l2_hint; };
+// phase id per cell; the kernel stages the ids of its extended tile instead of the two fp64 modulus boxes and looks K, G
+// up in a 256-entry table in shared memory.  Same arithmetic on the same values, about 15 B less HBM traffic per
+// voxel-iteration and 96 fewer 128-byte lines through L2 per CTA step.  The ids are stored TILE-BLOCKED: for every
+// (tile, layer) the TX*TY ids of the extended tile are contiguous (halo ids duplicated, they never change), so one
+// plain 1-D cp.async.bulk of 512 B brings them; as a 16-row tensor box they cost as much as a whole fp64 box.
+// tensor maps of one launch: 0..3 = vx vy vz G, 4..10 = K sxx syy szz txy txz tyz (old state + moduli)
+struct DrTmaps {
+    CUtensorMap m[DR_TMA_NA + DR_TMA_NB];
+    const unsigned char* ids;       // [nz+3][gy][gx][TY][TX] phase ids (layer -1 first)
+    const double* pal;              // K[256], G[256]
+    int gx, gy;                     // tiles in x and y
+    unsigned long long l2_hint;
+};
 
 template <int TX, int TY, int PAL = 0>
 struct DrTmaCfg {
@@ -70,20 +78,26 @@ __device__ __forceinline__ void dr_tma_load_3d(void* dst, const CUtensorMap* map
         ::"r"(dr_smem_u32(dst)), "l"((unsigned long long)map), "r"(dr_smem_u32(bar)), "r"(x), "r"(y), "r"(z), "l"(hint) : "memory");
 }
 
+__device__ __forceinline__ void dr_bulk_load_1d(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dr_smem_u32(dst)), "l"((unsigned long long)src), "r"(bytes), "r"(dr_smem_u32(bar)) : "memory");
+}
+
 // one batch: ring-A fields of layer m (z = m+1 in the padded box) and, if with_b, the ring-B set m:
 //   FORM 0: K, sigma_xx, sigma_yy, sigma_zz, tau_xy of layer m-1 and tau_xz, tau_yz of face m
 //   FORM 1: K, w_x, w_y, w_z of layer m-1 (w lives in the sigma_aa slots of the state buffer)
 template <int FORM, int PAL, int TX, int TY>
 __device__ __forceinline__ void dr_tma_issue_batch(const DrTmaps& T, unsigned long long* bar, double* da, double* db,
-                                                   unsigned char* idd, int x0, int xa, int y0, int m, bool with_b) {
+                                                   unsigned char* idd, const unsigned char* idsrc, long long idstride,
+                                                   int x0, int y0, int m, bool with_b) {
     constexpr int PL = TX * TY;
-    constexpr unsigned BA = 3 * PL * sizeof(double) + (PAL ? DR_ID_ROW * TY : PL * sizeof(double));
+    constexpr unsigned BA = 3 * PL * sizeof(double) + (PAL ? PL : PL * sizeof(double));
     constexpr unsigned BB = ((FORM ? 3 : 6) + (PAL ? 0 : 1)) * PL * sizeof(double);
     constexpr int BK = PAL ? 0 : 1;
     dr_mbar_expect_tx(bar, with_b ? BA + BB : BA);
 #pragma unroll
     for (int f = 0; f < 3; ++f) dr_tma_load_3d(da + f * PL, &T.m[f], bar, x0, y0, m + 1, T.l2_hint);
-    if (PAL) dr_tma_load_3d(idd, &T.mid, bar, xa, y0, m + 1, T.l2_hint);
+    if (PAL) dr_bulk_load_1d(idd, idsrc + idstride * (m + 1), PL, bar);
     else     dr_tma_load_3d(da + 3 * PL, &T.m[3], bar, x0, y0, m + 1, T.l2_hint);
     if (with_b) {
         if (!PAL) dr_tma_load_3d(db, &T.m[4], bar, x0, y0, m, T.l2_hint);                   // K of layer m-1
@@ -112,7 +126,8 @@ struct DrTmaCfg2 : DrTmaCfg<TX, TY, PAL> {
 
 template <int GAVG, int RES, int FORM, int PAL, int TX, int TY, bool BND, int PAR>
 __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, const DrTmaps& T, const DrFusedPtrs& g,
-                                            double* sm, unsigned char* idr, const double* pal, const int sid, const int xa,
+                                            double* sm, unsigned char* idr, const double* pal, const unsigned char* idsrc,
+                                            const long long idstride,
                                             unsigned long long* bars, const int s, const int t, const int k,
                                             const int kb, const int ke, const bool store, const int i, const int j,
                                             const int x0, const int y0, const bool producer, const bool midrow, const bool inner,
@@ -125,12 +140,12 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
     const double* Ac = sm + Cfg::RING_A + (t & 3) * (Cfg::NA * PL) + s;            // layer k
     const double* An = sm + Cfg::RING_A + ((t + 1) & 3) * (Cfg::NA * PL) + s;      // layer k+1
     const double* Bs = sm + Cfg::RING_B + (t % 3) * (Cfg::NB * PL) + s;            // set k+1
-    const unsigned char* Ic = idr + (t & 3) * (DR_ID_ROW * TY) + sid;               // phase ids of layer k   (PAL)
-    const unsigned char* In = idr + ((t + 1) & 3) * (DR_ID_ROW * TY) + sid;         // phase ids of layer k+1 (PAL)
+    const unsigned char* Ic = idr + (t & 3) * PL + s;                               // phase ids of layer k   (PAL)
+    const unsigned char* In = idr + ((t + 1) & 3) * PL + s;                         // phase ids of layer k+1 (PAL)
     // moduli of the own cell and of its -x / -y neighbours: from the fp64 planes, or through the palette (pal[id] = K,
     // pal[256 + id] = G)
     auto Gof = [&](const double* A, const unsigned char* I, int dx, int dy) -> double {
-        return PAL ? pal[256 + I[dy * DR_ID_ROW + dx]] : A[3 * PL + dy * TX + dx];
+        return PAL ? pal[256 + I[dy * TX + dx]] : A[3 * PL + dy * TX + dx];
     };
     double* X = sm + Cfg::XCH + PAR * (X_COUNT * PL) + s;                           // this step's exchange planes
 
@@ -201,7 +216,7 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
         unsigned long long* bar = bars + (b & 3);
         double* da = sm + Cfg::RING_A + (b & 3) * (Cfg::NA * PL);
         double* db = sm + Cfg::RING_B + ((b - 1) % 3) * (Cfg::NB * PL);
-        dr_tma_issue_batch<FORM, PAL, TX, TY>(T, bar, da, db, idr + (b & 3) * (DR_ID_ROW * TY), x0, xa, y0, m, true);
+        dr_tma_issue_batch<FORM, PAL, TX, TY>(T, bar, da, db, idr + (b & 3) * PL, idsrc, idstride, x0, y0, m, true);
     }
     // ---- wait HERE for the batch of the next step (issued two steps ago), not at the top of the next step: stage B
     // below and stage A of the next step then form one straight-line region that the scheduler can interleave
@@ -278,8 +293,8 @@ __device__ __forceinline__ void dr_tma_step(const DrLayout& L, const DrPT& P, co
 
 template <int GAVG, int RES, int FORM, int PAL, int TX, int TY, bool BND>
 __device__ __forceinline__ void dr_tma_march(const DrLayout& L, const DrPT& P, const DrTmaps& T, const DrFusedPtrs& g,
-                                             double* sm, unsigned char* idr, const double* pal, const int sid, const int xa,
-                                             unsigned long long* bars, const int s, const int kb, const int ke,
+                                             double* sm, unsigned char* idr, const double* pal, const unsigned char* idsrc,
+                                             const long long idstride, unsigned long long* bars, const int s, const int kb, const int ke,
                                              const int i, const int j, const int x0, const int y0,
                                              const bool producer, const bool midrow, const bool inner, double& rmax, bool& rnan) {
     DrCarry fa, fb;
@@ -287,9 +302,9 @@ __device__ __forceinline__ void dr_tma_march(const DrLayout& L, const DrPT& P, c
     fb = fa;
     int k = kb - 1;
     for (int t = 0; k < ke; t += 2, k += 2) {
-        dr_tma_step<GAVG, RES, FORM, PAL, TX, TY, BND, 0>(L, P, T, g, sm, idr, pal, sid, xa, bars, s, t, k, kb, ke, k >= kb, i, j, x0, y0, producer, midrow, inner, fa, fb, rmax, rnan);
+        dr_tma_step<GAVG, RES, FORM, PAL, TX, TY, BND, 0>(L, P, T, g, sm, idr, pal, idsrc, idstride, bars, s, t, k, kb, ke, k >= kb, i, j, x0, y0, producer, midrow, inner, fa, fb, rmax, rnan);
         if (k + 1 < ke)
-            dr_tma_step<GAVG, RES, FORM, PAL, TX, TY, BND, 1>(L, P, T, g, sm, idr, pal, sid, xa, bars, s, t + 1, k + 1, kb, ke, true, i, j, x0, y0, producer, midrow, inner, fb, fa, rmax, rnan);
+            dr_tma_step<GAVG, RES, FORM, PAL, TX, TY, BND, 1>(L, P, T, g, sm, idr, pal, idsrc, idstride, bars, s, t + 1, k + 1, kb, ke, true, i, j, x0, y0, producer, midrow, inner, fb, fa, rmax, rnan);
     }
 }
 
@@ -298,7 +313,7 @@ __global__ void __launch_bounds__(TX * TY, 1)
 k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int lz, unsigned long long* res_bits) {
     extern __shared__ __align__(1024) double sm[];
     __shared__ __align__(8) unsigned long long bars[4];
-    __shared__ __align__(128) unsigned char idr_raw[PAL ? 128 + 4 * DR_ID_ROW * TY + 128 : 16];   // id ring + slack for -1 row reads
+    __shared__ __align__(128) unsigned char idr_raw[PAL ? 128 + 4 * TX * TY + 128 : 16];          // id ring + slack for -1 row reads
     __shared__ double pal[PAL ? 512 : 1];                                                          // K[256], G[256]
     unsigned char* idr = idr_raw + (PAL ? 128 : 0);
     using Cfg = DrTmaCfg2<TX, TY, PAL>;
@@ -310,8 +325,8 @@ k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int 
     const int kb = blockIdx.z * lz;                          // first output layer of this chunk
     const int ke = min(kb + lz, nz + 1);                     // one past the last output layer (layer nz = top faces)
     const int x0 = DR_OX + i0 - 1, y0 = j0;                  // box origin in padded-field coordinates (z = layer + 1)
-    const int xa = x0 & ~15;                                 // id box origin: 16-byte aligned (TMA), x0 - xa in {0,2,..,14}
-    const int sid = ty * DR_ID_ROW + (x0 - xa) + tx;         // own id inside an id slot
+    const long long idstride = (long long)T.gx * T.gy * (TX * TY);                                   // bytes per layer of ids
+    const unsigned char* idsrc = T.ids + ((long long)blockIdx.y * T.gx + blockIdx.x) * (TX * TY);   // this tile, layer -1
     const int s = ty * TX + tx;
     if (PAL) for (int e = s; e < 512; e += TX * TY) pal[e] = T.pal[e];
     const bool producer = (tx == 0 && ty == 0);
@@ -331,7 +346,7 @@ k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int 
                 unsigned long long* bar = bars + b;
                 double* da = sm + Cfg::RING_A + b * (Cfg::NA * PL);
                 double* db = sm + Cfg::RING_B + (b >= 1 ? b - 1 : 0) * (Cfg::NB * PL);
-                dr_tma_issue_batch<FORM, PAL, TX, TY>(T, bar, da, db, idr + b * (DR_ID_ROW * TY), x0, xa, y0, m, b >= 1);
+                dr_tma_issue_batch<FORM, PAL, TX, TY>(T, bar, da, db, idr + b * PL, idsrc, idstride, x0, y0, m, b >= 1);
             }
         }
     }
@@ -347,8 +362,8 @@ k_pt_tma(const __grid_constant__ DrTmaps T, DrLayout L, DrPT P, DrFields B, int 
     double rmax = 0.0;
     bool rnan = false;
     const bool interior = i0 >= 2 && i0 + TX - 2 <= nx - 1 && j0 >= 2 && j0 + TY - 2 <= ny - 1;
-    if (interior) dr_tma_march<GAVG, RES, FORM, PAL, TX, TY, false>(L, P, T, g, sm, idr, pal, sid, xa, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
-    else          dr_tma_march<GAVG, RES, FORM, PAL, TX, TY, true>(L, P, T, g, sm, idr, pal, sid, xa, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
+    if (interior) dr_tma_march<GAVG, RES, FORM, PAL, TX, TY, false>(L, P, T, g, sm, idr, pal, idsrc, idstride, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
+    else          dr_tma_march<GAVG, RES, FORM, PAL, TX, TY, true>(L, P, T, g, sm, idr, pal, idsrc, idstride, bars, s, kb, ke, i, j, x0, y0, producer, midrow, inner, rmax, rnan);
 
     if (RES) {
         __shared__ unsigned long long smr[32];

@@ -36,7 +36,9 @@ def test_workspace_bytes_host_logic(libdr):
     assert binding.workspace_bytes(1, 8, 8) == 0 and binding.workspace_bytes(8, 8, 0) == 0
     b32 = binding.workspace_bytes(32, 32, 32)
     # 22 padded boxes of PX x 35 x 35 doubles (+ small scratch); PX = 17 + 34 rounded up to 64, +16 off the 512 B pitch
-    assert 22 * 80 * 35 * 35 * 8 <= b32 <= 22 * 80 * 35 * 35 * 8 + 22 * 256 + 65536
+    # + tile-blocked uint8 phase ids: 2 x 3 tiles x 35 layers x 512 B
+    ids = 2 * 3 * 35 * 512
+    assert 22 * 80 * 35 * 35 * 8 + ids <= b32 <= 22 * 80 * 35 * 35 * 8 + ids + 22 * 256 + 131072
     assert binding.workspace_bytes(703, 703, 703) < 70e9          # config 5 fits one B200 (180 GB)
 
 
