@@ -34,8 +34,8 @@ from paper_2410_20441_b200 import inputs, shard  # noqa: E402
 
 BYTES_PER_VOXEL_ITER = 160.0        # (2*9 + 2) fp64, SURVEY 8(d)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_pt_tma at 479^3 from the one `ncu --set full` capture
-# summarised in profiles/r1_summary.md (10.96 + 7.99 GB); null for any other workload / kernel
-NCU_TRAFFIC_BYTES = {("cfg4", 0): 18.94e9}
+# summarised in profiles/r1_summary.md (8.96 + 7.95 GB with the phase ids, 10.96 + 7.99 GB with fp64 K, G); null for any other workload / kernel
+NCU_TRAFFIC_BYTES = {("cfg4", 0, 1): 16.91e9, ("cfg4", 0, 0): 18.94e9}      # (workload, kernel, palette)
 WORKLOADS = {
     "cfg1": dict(n=32, gen="config1_sphere", desc="32^3 centred spherical pore r=5, contrast 1e-6"),
     "cfg2": dict(n=191, gen="config2_spheroid", desc="191^3 oblate fluid spheroid (40,40,8)"),
@@ -311,7 +311,7 @@ def main():
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": {0: "k_pt_tma", 1: "k_stress_split+k_velocity_split", 2: "k_pt_fused"}[args.kernel],
                      "achieved": kern_gbs, "peak": peak, "unit": "GB/s", "frac": kern_gbs / peak,
-                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.kernel)) if (args.n is None and args.form == 0) else None, "peak_source": peak_src, "launch_ms": kms,
+                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.kernel, int(pal_active))) if (args.n is None and args.form == 0) else None, "peak_source": peak_src, "launch_ms": kms,
                      "algorithmic_bytes_per_launch": bpv * N},
     }
     if tts is not None:
