@@ -25,6 +25,10 @@
  * Table 4 (spheroid): geometry garbled at P:194 and shear-test BCs garbled at P:369 --
  * "parity unpinned" for the shear-test boundary rule beyond sign and size of its effect.
  *
+ * DRO_FORM = 1 selects the displacement form of the same discrete problem (state u, w; stresses = Hooke's law of u;
+ * w <- (1-theta) w + C~^2 h^2 F/H_node, u <- u + w): not in the paper's text (it cites the method family at P:78), kept
+ * because it has the same fixed point -- pinned by tests P10, P10b -- and is the oracle of libdr's DR_FORM = 1.
+ *
  * Grid (sec. 3.3, Fig. 1): nx*ny*nz cells of size h, x fastest.
  *   cells  (nx,ny,nz)      : p, txx, tyy, tzz, K, G     at ((i+.5)h,(j+.5)h,(k+.5)h)
  *   vx     (nx+1,ny,nz)    at (i h,(j+.5)h,(k+.5)h);  vy (nx,ny+1,nz);  vz (nx,ny,nz+1)
