@@ -361,10 +361,15 @@ def test_fuzz_random_shapes_and_parameters(oracle_mod, gpu, seed):
     """seeded random shapes (2..69 per axis), kernels, forms, boundary modes, chunkings, void/fluid cells"""
     rng = np.random.default_rng(1000 + seed)
     shape, params, lc, eps0, niter, h = _fuzz_case(rng)
-    K, G = inputs.random_smooth(shape, seed=seed)
-    m = rng.uniform(size=K.shape)
-    K[m < 0.05] = 0.0; G[m < 0.05] = 0.0          # void
-    G[(m > 0.05) & (m < 0.1)] = 0.0               # fluid
+    if seed % 2:                                  # every other case: few distinct (K,G) pairs -> phase-id path
+        K, G = _quantised(shape, int(rng.integers(2, 40)), seed)
+        if rng.uniform() < 0.3:
+            params["void_rel"] = 0.1
+    else:
+        K, G = inputs.random_smooth(shape, seed=seed)
+        m = rng.uniform(size=K.shape)
+        K[m < 0.05] = 0.0; G[m < 0.05] = 0.0          # void
+        G[(m > 0.05) & (m < 0.1)] = 0.0               # fluid
     if params.get("form") == 1:
         params.setdefault("st_factor", 0.5 if max(shape) < 12 else 1.0)      # keep theta well below 1 on tiny grids
         if max(shape) < 12:
