@@ -20,10 +20,14 @@
  * point; Backus layered medium = Table 2 analytic column; cubic symmetry of a
  * centred sphere; dilute Eshelby pore; Hashin-Shtrikman; Betti symmetry; Eq. 27-29
  * identity; axis permutation; independence of PT constants; dense linear solve of the
- * same discrete problem assembled independently in numpy (brute force, n <= 6).
- * Not pinned: closeness to the paper's own *numerical* column of Table 2 for C44/C55 and
- * Table 4 (spheroid): geometry garbled at P:194 and shear-test BCs garbled at P:369 --
- * "parity unpinned" for the shear-test boundary rule beyond sign and size of its effect.
+ * same discrete problem assembled independently in numpy (brute force, n <= 6); the survey's
+ * independent probe numbers incl. iteration counts -- these also
+ * cover mean4(gavg=1), the DRO_FORM=1 iterate and, with the zero-by-hand test, apply_void_clamp.
+ * Not pinned: closeness to the paper's own *numerical* column of Table 2 (C33 30.419, C44/C55 15.307,
+ * C66 25.376, C12 3.720, C13 2.148) and Table 4 (spheroid): geometry garbled at P:194 and
+ * shear-test BCs garbled at P:369 -- "parity unpinned" for readings R4/R5 against the paper's own code
+ * beyond sign and size of their effect.  A bounded experiment showed that none of
+ * the documented readings (gavg 0/1 x bc_mode 0/1) reproduces that column to its printed decimals.
  *
  * DRO_FORM = 1 selects the displacement form of the same discrete problem (state u, w; stresses = Hooke's law of u;
  * w <- (1-theta) w + C~^2 h^2 F/H_node, u <- u + w): not in the paper's text (it cites the method family at P:78), kept

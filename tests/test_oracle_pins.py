@@ -368,6 +368,84 @@ def test_bruteforce_h_not_one_noncubic(oracle_mod):
         assert np.max(np.abs(col - cb)) <= 1e-8 * np.max(np.abs(cb))
 
 
+# ---------------------------------------------------------------- P14c/d/e: the branches round 1 left unpinned
+def test_P14c_arithmetic_G_config1_matches_survey_probe(oracle_mod):
+    """gavg = 1 (arithmetic 4-cell mean, reading R4 alternative) against SURVEY App. B4: the residual plateaus,
+    the survey's values were 'reached by ~650 its' and are printed to 5 decimals."""
+    g = read_golden("survey_probe_B.txt")["B4_config1_arithmetic_G"]
+    K, G, _ = inputs.config1_sphere()
+    o = oracle_mod.Oracle(K, G, gavg=1)
+    o.step(0, 1e-4, int(g[3]))
+    c0 = o.avg_stress() / 1e-4
+    o.step(3, 1e-4, int(g[4]))
+    c3 = o.avg_stress() / 1e-4
+    assert abs(c0[0] - g[0]) <= 1e-5 * g[0] and abs(c0[1] - g[1]) <= 1e-5 * g[0] and abs(c3[3] - g[2]) <= 1e-5 * g[0]
+    # and it is NOT the harmonic result (B3): the branch is really taken
+    h = read_golden("survey_probe_B.txt")["B3_config1_sphere_r5_32"]
+    assert abs(c0[0] - h[0]) > 0.5 and abs(c3[3] - h[2]) > 0.1
+
+
+@pytest.mark.parametrize("gavg", [0, 1])
+def test_P14d_layered_shear_C55_matches_survey_probe(oracle_mod, gavg):
+    """the paper's layered medium on 191 x 2 x 191, lc 4, tol 1e-7:
+    C55 = 14.70552 (harmonic) / 15.10604 (arithmetic), 2200 iterations.  Pins mean4 in both branches on an
+    interface-dominated case, the shear-test ghost rule, and the iteration count."""
+    g = read_golden("survey_probe_B.txt")["B9_layered_191x2x191_lc4"]
+    K, G, _ = inputs.layered(191, 2, 191)
+    o = oracle_mod.Oracle(K, G, gavg=gavg)
+    assert o.solve(4, 1e-4, 1e-7, 40000) == 0
+    assert abs(o.avg_stress()[4] / 1e-4 - g[gavg]) <= 2e-6 * g[gavg]
+    assert o.info()[0] == int(g[3])
+
+
+def test_P14e_displacement_form_iterate_matches_survey_probe(oracle_mod):
+    """the displacement form at the default C~ = 0.55 stops after 450 iterations on config 1
+    with the C of B3: pins the per-iteration constants of DRO_FORM = 1 ((1 - theta) damping, c2/H_node) through the
+    iteration count, not only through the fixed point."""
+    g = read_golden("survey_probe_B.txt")["B16_config1_displacement_form"]
+    K, G, _ = inputs.config1_sphere()
+    o = oracle_mod.Oracle(K, G, form=1)
+    o.set_param("cfl", 0.55)                  # DRO_FORM resets C~ to 0.50; the probe ran at 0.55
+    assert o.solve(0, 1e-4, 1e-8, 3200) == 0
+    assert o.info()[0] == int(g[3])
+    assert abs(o.avg_stress()[0] / 1e-4 - g[0]) <= 1e-6 * g[0]
+    assert o.solve(3, 1e-4, 1e-8, 3200) == 0
+    assert abs(o.avg_stress()[3] / 1e-4 - g[2]) <= 1e-6 * g[0]
+    # the damping constant matters: with (1 - theta/2) it would need a different number of iterations; a cheap
+    # cross-check that the count is sensitive is the form's own default C~ = 0.50 -> 500 iterations
+    o2 = oracle_mod.Oracle(K, G, form=1)
+    assert o2.solve(0, 1e-4, 1e-8, 3200) == 0 and o2.info()[0] == 500
+
+
+def test_void_clamp_equals_zeroing_that_phase_by_hand(oracle_mod):
+    """apply_void_clamp: three-phase image, void_rel chosen so that exactly ONE phase (the softest) is at or below the
+    threshold r * max(K + 4G/3): every field after 40 iterations equals, bit for bit, the run on the image with that
+    phase set to K = G = 0 by hand.  A threshold on K alone, '<' for '<=', or clamping the wrong phase fails."""
+    rng = np.random.default_rng(21)
+    ph = rng.integers(0, 3, size=(7, 9, 8))
+    # phase 2 sits EXACTLY on the threshold (K + 4G/3 = 0.01 * max): '<=' clamps it.  Phase 1 has a small K but a
+    # P-wave modulus above the threshold: a rule that looked at K alone would clamp it too.
+    Hmax = 60.0 + 4 * 30.0 / 3
+    Kt = np.array([60.0, 0.5, 0.4]); Gt = np.array([30.0, 20.0, (0.01 * Hmax - 0.4) * 0.75])
+    assert abs(Kt[2] + 4 * Gt[2] / 3 - 0.01 * Hmax) < 1e-15 and Kt[1] + 4 * Gt[1] / 3 > 0.01 * Hmax
+    K, G = Kt[ph], Gt[ph]
+    Kz, Gz = K.copy(), G.copy()
+    Kz[ph == 2] = 0.0; Gz[ph == 2] = 0.0
+    thr = float(Kt[2] + 4 * Gt[2] / 3) / Hmax          # the same floating-point quotient the rule multiplies back
+    a = oracle_mod.Oracle(K, G, void_rel=thr)
+    b = oracle_mod.Oracle(Kz, Gz)
+    c = oracle_mod.Oracle(K, G)
+    for lc in (0, 4):
+        a.step(lc, 1e-4, 40); b.step(lc, 1e-4, 40); c.step(lc, 1e-4, 40)
+        for f in range(9):
+            assert np.array_equal(a.get_field(f), b.get_field(f)), (lc, f)
+        assert not np.array_equal(a.get_field(0), c.get_field(0))          # and the clamp did something
+    # just below the threshold nothing is clamped
+    d = oracle_mod.Oracle(K, G, void_rel=thr * (1 - 1e-12))
+    d.step(0, 1e-4, 40); c.step(0, 1e-4, 40)
+    assert np.array_equal(d.get_field(0), c.get_field(0))
+
+
 # ---------------------------------------------------------------- ABI behaviour
 def test_argument_checks(oracle_mod):
     K, G = inputs.homogeneous(3)
