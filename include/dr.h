@@ -20,6 +20,8 @@
  *  - Units of C* are the units of K and G.
  *  - The library allocates NO device memory: the caller passes one workspace of dr_workspace_bytes() bytes
  *    (e.g. a torch tensor) that is borrowed until dr_destroy.  K and G are borrowed during dr_create only.
+ *  - A handle belongs to the CUDA device that was current at dr_create (the device of the workspace and the stream);
+ *    every call switches to it and restores the caller's device on return.
  *  - Every launch goes to the cuda_stream given at dr_create (a cudaStream_t cast to void*, NULL = default
  *    stream).  Calls that return host values synchronise that stream.
  *  - Errors are return codes, never exceptions or aborts.  dr_last_error() gives a message for the last
@@ -57,16 +59,35 @@ typedef enum {
     DR_VOID_REL = 4,   /* r>0: cells with K+4G/3 <= r*max(K+4G/3) become exact void K=G=0 [0 = off] (R9)      */
     DR_BC_MODE = 5,    /* 0 paper's mixed BCs [default]; 1 full kinematic uniform BC on all faces (R5)        */
     DR_KERNEL = 6,     /* 0 fused z-march kernel with TMA staging [default]; 1 split stress/velocity kernels
-                          (baseline); 2 fused z-march kernel with register-prefetched LDG loads              */
+                          (baseline); 2 fused z-march kernel with register-prefetched LDG loads;
+                          3 temporal blocking: TWO PT iterations per sweep (the state is read and written once per two
+                          iterations) on stencil-coded images -- images with <= 256 distinct (K,G) pairs, edge moduli
+                          and node stiffnesses, i.e. segmented rock images; other images, odd leftovers and a check
+                          iteration that is the first of a pair run kernel 0 (dr_active_kernel tells); stress form only;
+                          4 one iteration per sweep with the coded kernel (A/B reference of 3)                          */
     DR_ZCHUNK = 7,     /* z layers per CTA of the fused kernels; 0 = automatic [default] (tuning knob)            */
     DR_PALETTE = 9,    /* 1 [default]: images with <= 256 distinct (K,G) pairs run the fused kernel on a uint8 phase id
                           per cell and a 256-entry table instead of the two fp64 modulus fields (same values, 14 B less
                           HBM traffic per voxel-iteration); 0: always the fp64 modulus fields                        */
+    DR_STAG_TOL = 10,  /* second stopping rule of dr_solve (Reading R9b; the paper gives no rule beyond P:78): at every residual
+                          check with res > tol the volume averages <sigma> (Eq. 7) are formed; two consecutive checks that
+                          moved them by <= stag_tol (relative, max-norm over the 6 components) end the solve with DR_OK and
+                          dr_stop_reason() = DR_STOP_STAGNATION [1e-10; 0 = off].  It ends solves whose max-norm plateaus
+                          in near-void pores (contrast 1e-6) while C* is converged; DR_VOID_REL stays opt-in because
+                          it changes the moduli                                                                          */
     DR_FORM = 8        /* 0 stress-relaxation form of the paper, Eq. 11-13 [default]; 1 displacement form: state u, w,
                           w <- (1-theta) w + C~^2 h^2 F(u)/H_node, u <- u + w, stresses formed on the fly (same fixed
                           point, 112 instead of 160 B per voxel-iteration; DR_KERNEL 0 or 1).  Setting DR_FORM also resets
                           DR_CFL to the form's default (0.55 / 0.50: the explicit damping has less stability margin) */
 } dr_param;
+
+/* which rule ended the last dr_solve on a handle (dr_stop_reason) */
+typedef enum {
+    DR_STOP_NONE = 0,        /* no solve yet, or the solve diverged                                   */
+    DR_STOP_RESIDUAL = 1,    /* res <= tol                                                       */
+    DR_STOP_STAGNATION = 2,  /* <sigma> stopped moving between residual checks (DR_STAG_TOL)            */
+    DR_STOP_MAXITER = 3      /* neither: maxiter reached (status DR_MAXITER)                            */
+} dr_stop;
 
 /* Bytes of device workspace dr_create needs for an nx*ny*nz grid (0 if the sizes are invalid). */
 size_t dr_workspace_bytes(int nx, int ny, int nz);
@@ -82,12 +103,15 @@ dr_status dr_create(int nx, int ny, int nz, double h,
                     void* workspace, size_t workspace_bytes,
                     void* cuda_stream, dr_handle** out);
 
-/* Set a parameter (before dr_solve / dr_step). */
+/* Set a parameter (before dr_solve / dr_step).  Changing a parameter that shapes the iterate (DR_CFL, DR_ST_FACTOR,
+ * DR_GAVG, DR_VOID_REL, DR_BC_MODE, DR_KERNEL, DR_FORM) discards the current fields: dr_iterate / dr_get_field return
+ * DR_ERR_STATE until the next dr_step / dr_solve. */
 dr_status dr_set_param(dr_handle* h, int id, double value);
 
 /* One load case: initial fields and boundary values (App. A), then PT iterations (Eq. 11-13) until the
  * residual max-norm  res = max_nodes |div sigma| h / (H_node |eps0|)  <= tol, tested every ncheck iterations
- * ("once the dynamic fields attenuate to a certain precision"), at most maxiter iterations; then the
+ * ("once the dynamic fields attenuate to a certain precision"), or until <sigma> has stopped moving
+ * (DR_STAG_TOL), at most maxiter iterations; then the
  * volume averages (Eq. 7) and column load_case of C* (Eq. 9, 22).  eps0 != 0, tol > 0, maxiter >= 1. */
 dr_status dr_solve(dr_handle* h, int load_case, double eps0, double tol, int maxiter);
 
@@ -145,6 +169,13 @@ dr_status dr_contribution_tensor(const double C_eff[36], const double C_matrix[3
 /* 1 if dr_solve / dr_step on this handle run the phase-id (palette) variant of the fused kernel (the image has at
  * most 256 distinct (K,G) pairs, DR_PALETTE = 1, DR_KERNEL = 0), else 0. */
 int dr_uses_palette(dr_handle* h);
+
+/* Kernel the iterations on this handle run with the current parameters and image (see DR_KERNEL; valid after
+ * dr_step / dr_solve).  -1 for a NULL handle. */
+int dr_active_kernel(dr_handle* h);
+
+/* dr_stop value of the last dr_solve / dr_solve_six on this handle: which stopping rule fired. */
+int dr_stop_reason(dr_handle* h);
 
 /* Number of kernel launches this handle has issued so far (for bench.py's gpu_launches). */
 long long dr_launch_count(dr_handle* h);

@@ -56,7 +56,8 @@ extern "C" {
 enum { DRO_OK = 0, DRO_ERR_ARG = 1, DRO_ERR_WORKSPACE = 2, DRO_ERR_CUDA = 3,
        DRO_ERR_DIVERGED = 4, DRO_ERR_STATE = 5, DRO_MAXITER = 6 };
 enum { DRO_CFL = 0, DRO_ST_FACTOR = 1, DRO_NCHECK = 2, DRO_GAVG = 3,
-       DRO_VOID_REL = 4, DRO_BC_MODE = 5, DRO_FORM = 8 };
+       DRO_VOID_REL = 4, DRO_BC_MODE = 5, DRO_FORM = 8, DRO_STAG_TOL = 10 };
+enum { DRO_STOP_NONE = 0, DRO_STOP_RESIDUAL = 1, DRO_STOP_STAGNATION = 2, DRO_STOP_MAXITER = 3 };
 
 struct dro_handle {
     int nx, ny, nz;
@@ -65,6 +66,8 @@ struct dro_handle {
     std::vector<double> K, G;        /* after the optional void clamp              */
     /* parameters */
     double cfl, st_factor, void_rel;
+    double stag_tol;                 /* second stopping rule (reading R9b); 0 = off */
+    int stop_reason;                 /* DRO_STOP_* of the last dro_solve */
     int ncheck, gavg, bc_mode;
     int form;                        /* 0 stress-relaxation form of the paper (Eq. 11-13); 1 displacement form */
     /* state */
@@ -411,6 +414,7 @@ int dro_create(int nx, int ny, int nz, double h, const double* K, const double* 
     H->nx = nx; H->ny = ny; H->nz = nz; H->h = h;
     H->K0.assign(K, K + N); H->G0.assign(G, G + N);
     H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->form = 0;
+    H->stag_tol = 1e-10; H->stop_reason = DRO_STOP_NONE;
     for (int a = 0; a < 6; ++a) { H->have[a] = false; for (int b = 0; b < 6; ++b) H->Ccol[a][b] = 0.0; }
     H->have_avg = false; H->iters = 0; H->residual = 0.0; H->ms = 0.0;
     *out = H;
@@ -429,13 +433,21 @@ int dro_set_param(dro_handle* H, int id, double value) {
         /* the explicit damping of the displacement form has a smaller stability margin (diverges at C~ = 0.55 on
            small grids, converges at 0.52): choosing a form also resets C~ to that form's default */
         case DRO_FORM:      if (value != 0.0 && value != 1.0) break; H->form = (int)value; H->cfl = H->form ? 0.50 : 0.55; return DRO_OK;
+        case DRO_STAG_TOL:  if (!(value >= 0.0)) break; H->stag_tol = value; return DRO_OK;
         default: break;
     }
     H->err = "bad parameter id or value";
     return DRO_ERR_ARG;
 }
 
-/* O7.3: iterate; every ncheck iterations test res <= tol. */
+/* O7.3: iterate; every ncheck iterations test res <= tol ("once the dynamic fields attenuate to a certain
+ * precision").
+ * Second rule (reading R9b in DESIGN.md; the paper states no stopping rule beyond P:78): with tiny-but-non-zero pore
+ * moduli the max-norm plateaus in the pores (H_node ~ 1e-6 of the matrix) while <sigma>, the only thing Eq. 9/22 use,
+ * no longer moves.  So at every check where res > tol the volume averages (O8) are formed and compared with those of
+ * the previous check: d = max_m |<sigma_m> - <sigma_m>_prev| / max_m |<sigma_m>|.  Two consecutive checks with
+ * d <= stag_tol (default 1e-10, four orders below the 1e-6 bar on C) stop the solve with DRO_OK and
+ * stop_reason = DRO_STOP_STAGNATION.  stag_tol = 0 switches the rule off. */
 int dro_solve(dro_handle* H, int lc, double eps0, double tol, int maxiter) {
     if (bad_solve_args(H, lc, eps0)) return DRO_ERR_ARG;
     if (!(tol > 0.0) || maxiter < 1) { H->err = "bad tol or maxiter"; return DRO_ERR_ARG; }
@@ -443,14 +455,27 @@ int dro_solve(dro_handle* H, int lc, double eps0, double tol, int maxiter) {
     init_fields(H, lc, eps0);
     int status = DRO_MAXITER;
     H->residual = INFINITY;
+    H->stop_reason = DRO_STOP_MAXITER;
+    bool have_prev = false;
+    double prev[6] = {0, 0, 0, 0, 0, 0};
+    int calm = 0;
     int it = 0;
     for (it = 1; it <= maxiter; ++it) {
         bool chk = (it % H->ncheck == 0);
         double r = pt_iteration(H, lc, eps0, chk);
         if (chk) {
             H->residual = r;
-            if (!std::isfinite(r)) { status = DRO_ERR_DIVERGED; break; }
-            if (r <= tol) { status = DRO_OK; break; }
+            if (!std::isfinite(r)) { status = DRO_ERR_DIVERGED; H->stop_reason = DRO_STOP_NONE; break; }
+            if (r <= tol) { status = DRO_OK; H->stop_reason = DRO_STOP_RESIDUAL; break; }
+            if (H->stag_tol > 0.0) {
+                double a[6], num = 0.0, den = 0.0;
+                volume_averages(H, a);
+                for (int m = 0; m < 6; ++m) { num = std::max(num, std::fabs(a[m] - prev[m])); den = std::max(den, std::fabs(a[m])); }
+                if (have_prev && num <= H->stag_tol * den) ++calm; else calm = 0;
+                for (int m = 0; m < 6; ++m) prev[m] = a[m];
+                have_prev = true;
+                if (calm >= 2) { status = DRO_OK; H->stop_reason = DRO_STOP_STAGNATION; break; }
+            }
         }
     }
     H->iters = std::min(it, maxiter);
@@ -459,6 +484,8 @@ int dro_solve(dro_handle* H, int lc, double eps0, double tol, int maxiter) {
     store_column(H, lc, eps0);
     return status;
 }
+
+int dro_stop_reason(dro_handle* H) { return H ? H->stop_reason : DRO_STOP_NONE; }
 
 /* fixed iteration count (parity): init, niter iterations, residual of the last one, averages. */
 int dro_step(dro_handle* H, int lc, double eps0, int niter) {

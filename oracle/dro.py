@@ -19,6 +19,8 @@ _LIB = os.path.join(_HERE, "libdro.so")
 OK, ERR_ARG, ERR_WORKSPACE, ERR_CUDA, ERR_DIVERGED, ERR_STATE, MAXITER = range(7)
 CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE = range(6)
 FORM = 8
+STAG_TOL = 10
+STOP_NONE, STOP_RESIDUAL, STOP_STAGNATION, STOP_MAXITER = range(4)
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
 
 
@@ -52,6 +54,7 @@ def lib():
         L.dro_get_field.argtypes = [C.c_void_p, C.c_int, dp, C.c_size_t]
         L.dro_last_error.argtypes = [C.c_void_p]
         L.dro_last_error.restype = C.c_char_p
+        L.dro_stop_reason.argtypes = [C.c_void_p]
         L.dro_destroy.argtypes = [C.c_void_p]
         L.dro_destroy.restype = None
         _lib = L
@@ -89,7 +92,7 @@ class Oracle:
         return st
 
     def set_param(self, name, value):
-        ids = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, form=FORM)
+        ids = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, form=FORM, stag_tol=STAG_TOL)
         self._check(lib().dro_set_param(self._h, ids[name], float(value)))
 
     def solve(self, lc, eps0=1e-4, tol=1e-8, maxiter=100000):
@@ -117,6 +120,9 @@ class Oracle:
         ms = C.c_double()
         lib().dro_info(self._h, C.byref(it), C.byref(r), C.byref(ms))
         return it.value, r.value, ms.value
+
+    def stop_reason(self):
+        return lib().dro_stop_reason(self._h)
 
     def field_shape(self, f):
         nx, ny, nz = self.nx, self.ny, self.nz

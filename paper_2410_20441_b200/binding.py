@@ -13,12 +13,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("DR_LIB") or os.path.join(_HERE, "libdr.so")     # DR_LIB: an alternative build (A/B timing)
 
 OK, ERR_ARG, ERR_WORKSPACE, ERR_CUDA, ERR_DIVERGED, ERR_STATE, MAXITER = range(7)
-CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK, FORM, PALETTE = range(10)
-PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK, form=FORM, palette=PALETTE)
+CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK, FORM, PALETTE, STAG_TOL = range(11)
+STOP_NONE, STOP_RESIDUAL, STOP_STAGNATION, STOP_MAXITER = range(4)
+PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK, form=FORM, palette=PALETTE, stag_tol=STAG_TOL)
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
 EXPORTS = ("dr_workspace_bytes", "dr_create", "dr_set_param", "dr_solve", "dr_solve_six", "dr_effective_C_six", "dr_step", "dr_iterate",
            "dr_effective_C", "dr_avg_stress", "dr_info", "dr_get_field", "dr_solve_image_host", "dr_contribution_tensor",
-           "dr_uses_palette", "dr_launch_count", "dr_last_error", "dr_destroy")
+           "dr_uses_palette", "dr_active_kernel", "dr_stop_reason", "dr_launch_count", "dr_last_error", "dr_destroy")
 
 _lib = None
 
@@ -52,6 +53,10 @@ def lib():
             L.dr_contribution_tensor.argtypes = [dp, dp, C.c_double, dp]
         if hasattr(L, "dr_uses_palette"):
             L.dr_uses_palette.argtypes = [vp]
+        if hasattr(L, "dr_active_kernel"):
+            L.dr_active_kernel.argtypes = [vp]
+        if hasattr(L, "dr_stop_reason"):
+            L.dr_stop_reason.argtypes = [vp]
         L.dr_launch_count.argtypes = [vp]
         L.dr_launch_count.restype = C.c_longlong
         L.dr_last_error.argtypes = [vp]
@@ -87,8 +92,6 @@ class Solver:
             raise RuntimeError("libdr needs a CUDA device (there is no CPU fallback)")
         if not (K.is_cuda and G.is_cuda and K.dtype == torch.float64 and G.dtype == torch.float64):
             raise TypeError("K and G must be float64 CUDA tensors")
-        K = K.contiguous()
-        G = G.contiguous()
         assert K.dim() == 3 and K.shape == G.shape
         self.nz, self.ny, self.nx = (int(s) for s in K.shape)
         self.device = K.device
@@ -101,7 +104,12 @@ class Solver:
         self.workspace = workspace
         self.stream = stream if stream is not None else torch.cuda.current_stream(K.device)
         self._h = C.c_void_p()
-        with torch.cuda.device(K.device):
+        # dr_create reads K, G on self.stream: order it behind whatever produced them on the caller's current stream,
+        # and make any contiguous() copy on self.stream too
+        self.stream.wait_stream(torch.cuda.current_stream(K.device))
+        with torch.cuda.device(K.device), torch.cuda.stream(self.stream):
+            K = K.contiguous()
+            G = G.contiguous()
             st = lib().dr_create(self.nx, self.ny, self.nz, float(h), K.data_ptr(), G.data_ptr(),
                                  workspace.data_ptr(), workspace.numel() * workspace.element_size(),
                                  self.stream.cuda_stream, C.byref(self._h))
@@ -150,6 +158,12 @@ class Solver:
         out = self._torch.empty(field_shape(self.nx, self.ny, self.nz, f), dtype=self._torch.float64, device=self.device)
         self._check(lib().dr_get_field(self._h, f, out.data_ptr(), out.numel()))
         return out
+
+    def stop_reason(self):
+        return lib().dr_stop_reason(self._h)
+
+    def active_kernel(self):
+        return lib().dr_active_kernel(self._h)
 
     def uses_palette(self):
         return bool(lib().dr_uses_palette(self._h))

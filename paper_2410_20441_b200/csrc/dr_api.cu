@@ -15,6 +15,7 @@
 #include "dr_kernels_split.cuh"
 #include "dr_kernels_fused.cuh"
 #include "dr_kernels_tma.cuh"
+#include "dr_kernels_tb2.cuh"
 
 #ifndef FUSED_TX
 #define FUSED_TX 32
@@ -39,11 +40,13 @@ struct dr_handle {
     int use_pal;                // DR_PALETTE
     unsigned int* flags;
     // host
-    double* pinned;             // 8 doubles, page-locked
+    double* pinned;             // 16 doubles, page-locked: [0..5] averages, [8] residual, [9..14] averages at a check
     cudaEvent_t e0, e1;
     // parameters
-    double cfl, st_factor, void_rel;
+    double cfl, st_factor, void_rel, stag_tol;
     int ncheck, gavg, bc_mode, kernel, form;
+    int device;                 // CUDA device of the workspace and the stream (every entry point switches to it)
+    int stop_reason;            // dr_stop: which rule ended the last dr_solve
     double void_applied;        // void_rel currently baked into K,G
     double hmax;
     // state
@@ -63,6 +66,16 @@ struct dr_handle {
     int fused_lz;
     CUtensorMap tm_state[2][F_COUNT];   // TMA descriptors of the padded boxes (both ping-pong buffers)
     CUtensorMap tm_K, tm_G;
+    // stencil-coded path (DR_KERNEL 3 / 4, dr_kernels_tb2.cuh)
+    unsigned long long* codes;  // [nz+5][gy2][gx2][TB2_TY][TB2_TX]
+    unsigned long long *ekeys, *rkeys;   // edge-modulus and 1/H_node tables (bit patterns), 256 each
+    double* tabs;               // TB2_TAB_N table values
+    bool has_codes;             // codes and tables are valid for (code_gavg, code_void)
+    bool codes_failed;          // more than 256 distinct edge / node values for that setting: one-sweep kernel instead
+    int code_gavg; double code_void;
+    int tb2_lz;
+    bool lz_user;               // DR_ZCHUNK set by the caller
+    CUtensorMap tm2_state[2][F_COUNT];   // boxes TB2_TX x TB2_TY x 1
     std::string err;
 };
 
@@ -76,6 +89,15 @@ static bool cuda_ok(dr_handle* H, cudaError_t e, const char* what) {
     if (H) H->err = std::string(what) + ": " + cudaGetErrorString(e);
     return false;
 }
+
+// every entry point runs on the device the handle was created on and restores the caller's device on return
+struct DrDeviceGuard {
+    int prev; bool sw;
+    explicit DrDeviceGuard(int dev) : prev(-1), sw(false) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) sw = (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~DrDeviceGuard() { if (sw) cudaSetDevice(prev); }
+};
 
 #define CK(call) do { if (!cuda_ok(H, (call), #call)) return DR_ERR_CUDA; } while (0)
 #define CKL(what) do { H->launches++; if (!cuda_ok(H, cudaGetLastError(), what)) return DR_ERR_CUDA; } while (0)
@@ -94,10 +116,18 @@ static int tiles_y(const DrLayout& L) { return (L.ny + 1 + FUSED_TY - 3) / (FUSE
 // tile-blocked phase ids: one FUSED_TX*FUSED_TY byte block per (tile, layer), layers -1 .. nz+1
 static size_t ids_bytes(const DrLayout& L) { return align_up((size_t)tiles_x(L) * tiles_y(L) * (L.nz + 3) * (FUSED_TX * FUSED_TY), 256); }
 
+static int tb2_tiles_x(const DrLayout& L) { return (L.nx + 2 + TB2_TX - 5) / (TB2_TX - 4); }     // owned columns start at i = -1
+static int tb2_tiles_y(const DrLayout& L) { return (L.ny + 1 + TB2_TY - 5) / (TB2_TY - 4); }
+// stencil codes: one 8-byte word per (tile, layer, thread), layers -TB2_KLO .. nz-1+TB2_KHI; + tables and their keys
+static size_t codes_bytes(const DrLayout& L) {
+    return align_up((size_t)tb2_tiles_x(L) * tb2_tiles_y(L) * (L.nz + TB2_KLO + TB2_KHI) * (TB2_TX * TB2_TY) * sizeof(unsigned long long), 256);
+}
+static const size_t CODE_SMALL_BYTES = 2 * 2048 + TB2_TAB_N * sizeof(double);
+
 extern "C" size_t dr_workspace_bytes(int nx, int ny, int nz) {
     if (!sizes_ok(nx, ny, nz)) return 0;
     DrLayout L = dr_make_layout(nx, ny, nz);
-    return (size_t)N_BIG * field_bytes(L) + ids_bytes(L) + SMALL_BYTES;
+    return (size_t)N_BIG * field_bytes(L) + ids_bytes(L) + SMALL_BYTES + codes_bytes(L) + CODE_SMALL_BYTES;
 }
 
 // z-chunk length of the fused kernels: make the CTA count fill whole waves of 148 SMs while keeping the priming
@@ -106,18 +136,23 @@ extern "C" size_t dr_workspace_bytes(int nx, int ny, int nz) {
 // (479^3: 3.53 ms/iteration at 24-32 layers per chunk, 3.67 at 48, 4.37 at 64, 5.2 at 96).
 #define DR_LZ_MAX 36
 #define DR_LZ_FIXED 3      // per-CTA start-up (barrier init, first TMA round trip) in units of one z step
-static int choose_lz(const DrLayout& L) {
-    const int tiles = ((L.nx + 1 + FUSED_TX - 3) / (FUSED_TX - 2)) * ((L.ny + 1 + FUSED_TY - 3) / (FUSED_TY - 2));
-    const int layers = L.nz + 1;
+static int choose_lz_for(int tiles, int layers, int priming) {
     int best_lz = layers < DR_LZ_MAX ? layers : DR_LZ_MAX;
     double best = 1e300;
     for (int lz = 1; lz <= DR_LZ_MAX && lz <= layers; ++lz) {
         const int chunks = (layers + lz - 1) / lz;
         const double waves = std::ceil((double)tiles * chunks / 148.0);
-        const double cost = waves * (lz + 1 + DR_LZ_FIXED);          // steps on the critical path of one SM
+        const double cost = waves * (lz + priming + DR_LZ_FIXED);          // steps on the critical path of one SM
         if (cost < best - 1e-9 || (cost < best + 1e-9 && lz > best_lz)) { best = cost; best_lz = lz; }
     }
     return best_lz;
+}
+static int choose_lz(const DrLayout& L) {
+    return choose_lz_for(tiles_x(L) * tiles_y(L), L.nz + 1, 1);
+}
+// the two-iteration kernel runs lz + 4 steps per chunk (two priming steps per iteration)
+static int choose_lz_tb2(const DrLayout& L) {
+    return choose_lz_for(tb2_tiles_x(L) * tb2_tiles_y(L), L.nz + 1, 4);
 }
 
 // TMA descriptor of one padded field: 3-D fp64 tensor (PX,PY,PZ), box (FUSED_TX, FUSED_TY, 1), no swizzle,
@@ -126,11 +161,11 @@ typedef CUresult (*dr_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, 
                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-static bool make_tmap(dr_handle* H, dr_encode_fn enc, CUtensorMap* out, double* base) {
+static bool make_tmap(dr_handle* H, dr_encode_fn enc, CUtensorMap* out, double* base, int bx = FUSED_TX, int by = FUSED_TY) {
     const DrLayout& L = H->L;
     cuuint64_t dims[3] = {(cuuint64_t)L.PX, (cuuint64_t)L.PY, (cuuint64_t)L.PZ};
     cuuint64_t strides[2] = {(cuuint64_t)L.PX * 8, (cuuint64_t)L.PX * L.PY * 8};
-    cuuint32_t box[3] = {FUSED_TX, FUSED_TY, 1};
+    cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1};
     cuuint32_t estr[3] = {1, 1, 1};
     const CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_NONE;   // 64/128/256 B measured: no difference
     CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -148,6 +183,7 @@ static bool make_all_tmaps(dr_handle* H) {
     }
     dr_encode_fn enc = (dr_encode_fn)fn;
     for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) if (!make_tmap(H, enc, &H->tm_state[b][f], H->buf[b][f])) return false;
+    for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) if (!make_tmap(H, enc, &H->tm2_state[b][f], H->buf[b][f], TB2_TX, TB2_TY)) return false;
     return make_tmap(H, enc, &H->tm_K, H->K) && make_tmap(H, enc, &H->tm_G, H->G);
 }
 
@@ -177,8 +213,15 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
     H->pal = (double*)p; p += 4096;
     p = (char*)align_up((size_t)p, 256);
     H->ids = (unsigned char*)p; p += ids_bytes(H->L);
+    H->codes = (unsigned long long*)p; p += codes_bytes(H->L);
+    H->ekeys = (unsigned long long*)p; p += 2048; H->rkeys = (unsigned long long*)p; p += 2048;
+    H->tabs = (double*)p; p += TB2_TAB_N * sizeof(double);
+    H->has_codes = false; H->codes_failed = false; H->code_gavg = -1; H->code_void = -1.0;
+    H->tb2_lz = choose_lz_tb2(H->L); H->lz_user = false;
     H->has_pal = false; H->use_pal = 1;
     H->pinned = nullptr; H->e0 = H->e1 = nullptr;
+    if (cudaGetDevice(&H->device) != cudaSuccess) { cudaGetLastError(); delete H; return DR_ERR_CUDA; }
+    H->stag_tol = 1e-10; H->stop_reason = DR_STOP_NONE;
     H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->kernel = 0; H->form = 0;
     H->void_applied = 0.0; H->hmax = 0.0;
     H->cur = 0; H->have_fields = false; H->cur_lc = -1; H->cur_eps0 = 0.0;
@@ -188,7 +231,7 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
 
     dr_status st = DR_OK;
     do {
-        if (!cuda_ok(H, cudaMallocHost((void**)&H->pinned, 8 * sizeof(double)), "cudaMallocHost")) { st = DR_ERR_CUDA; break; }
+        if (!cuda_ok(H, cudaMallocHost((void**)&H->pinned, 16 * sizeof(double)), "cudaMallocHost")) { st = DR_ERR_CUDA; break; }
         if (!cuda_ok(H, cudaEventCreate(&H->e0), "cudaEventCreate") || !cuda_ok(H, cudaEventCreate(&H->e1), "cudaEventCreate")) { st = DR_ERR_CUDA; break; }
         // state fields and moduli boxes start as zeros (halo nodes are never written afterwards)
         if (!cuda_ok(H, cudaMemsetAsync(workspace, 0, dr_workspace_bytes(nx, ny, nz), H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }
@@ -239,6 +282,14 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
         DR_SET_TMA_ATTR(0, 0, 1); DR_SET_TMA_ATTR(0, 1, 1); DR_SET_TMA_ATTR(1, 0, 1); DR_SET_TMA_ATTR(1, 1, 1);
 #undef DR_SET_TMA_ATTR
         if (!cuda_ok(H, e, "cudaFuncSetAttribute(k_pt_tma)")) { st = DR_ERR_CUDA; break; }
+        {
+            const int smem2 = (int)DrTb2Cfg<TB2_TX, TB2_TY>::SMEM;
+            e = cudaFuncSetAttribute(k_pt_tb2<0, 2, TB2_TX, TB2_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tb2<1, 2, TB2_TX, TB2_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tb2<0, 1, TB2_TX, TB2_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tb2<1, 1, TB2_TX, TB2_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
+            if (!cuda_ok(H, e, "cudaFuncSetAttribute(k_pt_tb2)")) { st = DR_ERR_CUDA; break; }
+        }
         if (!make_all_tmaps(H)) { st = DR_ERR_CUDA; break; }
     } while (0);
     if (st != DR_OK) {
@@ -254,19 +305,23 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
 
 extern "C" dr_status dr_set_param(dr_handle* H, int id, double v) {
     if (!H) return DR_ERR_ARG;
+    // parameters that shape the iterate invalidate the current fields: dr_iterate / dr_get_field then need a new
+    // dr_step / dr_solve (DR_ERR_STATE) instead of silently continuing on state built under the old value
     switch (id) {
-        case DR_CFL:       if (!(v > 0.0)) break; H->cfl = v; return DR_OK;
-        case DR_ST_FACTOR: if (!(v > 0.0)) break; H->st_factor = v; return DR_OK;
+        case DR_CFL:       if (!(v > 0.0)) break; H->cfl = v; H->have_fields = false; return DR_OK;
+        case DR_ST_FACTOR: if (!(v > 0.0)) break; H->st_factor = v; H->have_fields = false; return DR_OK;
         case DR_NCHECK:    if (!(v >= 1.0)) break; H->ncheck = (int)v; return DR_OK;
-        case DR_GAVG:      if (v != 0.0 && v != 1.0) break; H->gavg = (int)v; return DR_OK;
-        case DR_VOID_REL:  if (!(v >= 0.0)) break; H->void_rel = v; return DR_OK;
-        case DR_BC_MODE:   if (v != 0.0 && v != 1.0) break; H->bc_mode = (int)v; return DR_OK;
-        case DR_KERNEL:    if (v != 0.0 && v != 1.0 && v != 2.0) break; H->kernel = (int)v; return DR_OK;
+        case DR_GAVG:      if (v != 0.0 && v != 1.0) break; H->gavg = (int)v; H->have_fields = false; return DR_OK;
+        case DR_VOID_REL:  if (!(v >= 0.0)) break; H->void_rel = v; H->have_fields = false; return DR_OK;
+        case DR_BC_MODE:   if (v != 0.0 && v != 1.0) break; H->bc_mode = (int)v; H->have_fields = false; return DR_OK;
+        case DR_KERNEL:    if (v != 0.0 && v != 1.0 && v != 2.0 && v != 3.0 && v != 4.0) break; H->kernel = (int)v; H->have_fields = false; return DR_OK;
         // choosing a form also resets C~ to that form's default (the explicit damping of the displacement form
         // diverges at 0.55 on small grids)
         case DR_FORM:      if (v != 0.0 && v != 1.0) break; H->form = (int)v; H->cfl = H->form ? 0.50 : 0.55; H->have_fields = false; return DR_OK;
         case DR_PALETTE:   if (v != 0.0 && v != 1.0) break; H->use_pal = (int)v; return DR_OK;
-        case DR_ZCHUNK:    if (!(v >= 0.0) || v > 8192.0) break; H->fused_lz = v >= 1.0 ? (int)v : choose_lz(H->L); return DR_OK;
+        case DR_ZCHUNK:    if (!(v >= 0.0) || v > 8192.0) break;
+                           H->fused_lz = v >= 1.0 ? (int)v : choose_lz(H->L); H->tb2_lz = v >= 1.0 ? (int)v : choose_lz_tb2(H->L); return DR_OK;
+        case DR_STAG_TOL:  if (!(v >= 0.0)) break; H->stag_tol = v; return DR_OK;
         default: break;
     }
     return fail(H, DR_ERR_ARG, "bad parameter id or value");
@@ -300,6 +355,37 @@ static DrConstFields cfields_of(dr_handle* H, int b) {
     DrConstFields F; for (int f = 0; f < F_COUNT; ++f) F.f[f] = H->buf[b][f]; return F;
 }
 
+// stencil codes and tables of the coded path (dr_kernels_tb2.cuh) for the current DR_GAVG / DR_VOID_REL; an image with
+// more than 256 distinct (K,G) pairs, edge moduli or node stiffnesses is left uncoded (has_codes = false) and DR_KERNEL 3
+// then runs the one-sweep kernel
+static dr_status ensure_codes(dr_handle* H) {
+    if (!(H->has_pal && H->use_pal)) { H->has_codes = false; return DR_OK; }
+    if (H->code_gavg == H->gavg && H->code_void == H->void_applied) return DR_OK;      // built (or failed) for this setting
+    const DrLayout& L = H->L;
+    H->has_codes = false; H->codes_failed = false;
+    CK(cudaMemsetAsync(H->ekeys, 0xff, 4096, H->st));                                // ekeys and rkeys := EMPTY
+    CK(cudaMemsetAsync(H->flags, 0, 4, H->st));
+    dim3 blk(TB2_TX, TB2_TY, 1), grd(tb2_tiles_x(L), tb2_tiles_y(L), L.nz + TB2_KLO + TB2_KHI);
+#define DR_CODE(G_, P_) k_code_build<G_, P_><<<grd, blk, 0, H->st>>>(H->L, H->K, H->G, H->K0, H->G0, H->palK, H->palG, H->ekeys, H->rkeys, H->codes, H->flags)
+    if (H->gavg) DR_CODE(1, 0); else DR_CODE(0, 0);
+    CKL("k_code_build<0>");
+    unsigned int fl = 0;
+    CK(cudaMemcpyAsync(&fl, H->flags, 4, cudaMemcpyDeviceToHost, H->st));
+    CK(cudaStreamSynchronize(H->st));
+    H->code_gavg = H->gavg; H->code_void = H->void_applied;
+    if (fl & 8u) { H->codes_failed = true; return DR_OK; }
+    if (H->gavg) DR_CODE(1, 1); else DR_CODE(0, 1);
+    CKL("k_code_build<1>");
+#undef DR_CODE
+    k_code_tables<<<1, 256, 0, H->st>>>(H->pal, H->ekeys, H->rkeys, H->tabs);
+    CKL("k_code_tables");
+    CK(cudaMemcpyAsync(&fl, H->flags, 4, cudaMemcpyDeviceToHost, H->st));
+    CK(cudaStreamSynchronize(H->st));
+    if (fl & 16u) return fail(H, DR_ERR_CUDA, "stencil code lookup missed a table entry (internal error)");
+    H->has_codes = true;
+    return DR_OK;
+}
+
 static dr_status prepare(dr_handle* H, int lc, double eps0) {
     const DrLayout& L = H->L;
     if (H->void_applied != H->void_rel) {
@@ -307,6 +393,11 @@ static dr_status prepare(dr_handle* H, int lc, double eps0) {
         CKL("k_void_clamp");
         if (H->has_pal) { k_pal_values<<<1, 256, 0, H->st>>>(H->palK, H->palG, H->pal, H->void_rel * H->hmax); CKL("k_pal_values"); }
         H->void_applied = H->void_rel;
+    }
+    if (H->kernel >= 3) {
+        if (H->form == 1) return fail(H, DR_ERR_ARG, "DR_FORM = 1 is implemented by DR_KERNEL 0 and 1 only");
+        dr_status cs = ensure_codes(H);
+        if (cs != DR_OK) return cs;
     }
     DrPT P = make_pt(H, lc, eps0);
     dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
@@ -318,10 +409,37 @@ static dr_status prepare(dr_handle* H, int lc, double eps0) {
     return DR_OK;
 }
 
+// the coded kernels (DR_KERNEL 3, 4) need the stencil codes; without them the one-sweep TMA kernel runs
+static bool coded(const dr_handle* H) { return H->kernel >= 3 && H->has_codes && H->form == 0; }
+
+// nit PT iterations in one sweep of the coded kernel (dr_kernels_tb2.cuh); with_res: residual of the LAST of them
+static dr_status iteration_coded(dr_handle* H, const DrPT& P, bool with_res, int nit) {
+    const DrLayout& L = H->L;
+    const int lz = H->tb2_lz;
+    dim3 blk(TB2_TX, TB2_TY, 1), grd(tb2_tiles_x(L), tb2_tiles_y(L), (L.nz + 1 + lz - 1) / lz);
+    DrTb2Maps T;
+    const int c = H->cur;
+    static const int order[9] = {F_VX, F_VY, F_VZ, F_SXX, F_SYY, F_SZZ, F_TXY, F_TXZ, F_TYZ};
+    for (int f = 0; f < 9; ++f) T.m[f] = H->tm2_state[c][order[f]];
+    T.codes = H->codes; T.tabs = H->tabs; T.gx = (int)grd.x; T.gy = (int)grd.y;
+    T.l2_hint = 0x1000000000000000ull;
+    const size_t smem = DrTb2Cfg<TB2_TX, TB2_TY>::SMEM;
+    DrFields Bo = fields_of(H, c ^ 1);
+    if (nit == 2) { if (with_res) k_pt_tb2<1, 2, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(T, H->L, P, Bo, lz, H->res_bits);
+                    else          k_pt_tb2<0, 2, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); }
+    else          { if (with_res) k_pt_tb2<1, 1, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(T, H->L, P, Bo, lz, H->res_bits);
+                    else          k_pt_tb2<0, 1, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); }
+    CKL("k_pt_tb2");
+    H->cur ^= 1;
+    return DR_OK;
+}
+
 // one PT iteration; with_res: also accumulate the residual max-norm into res_bits (caller zeroes it)
 static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
     const DrLayout& L = H->L;
-    if (H->kernel == 1) {
+    if (H->kernel == 4 && coded(H)) return iteration_coded(H, P, with_res, 1);
+    const int kernel = H->kernel >= 3 ? 0 : H->kernel;      // DR_KERNEL 3 single sweeps, and uncoded images: the TMA kernel
+    if (kernel == 1) {
         dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
         // FORM 0: in place in buffer cur.  FORM 1: u, w in buffer cur, stresses of this iteration in buffer cur^1.
         DrFields U = fields_of(H, H->cur);
@@ -341,7 +459,7 @@ static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
     const int lz = H->fused_lz;
     dim3 blk(FUSED_TX, FUSED_TY, 1);
     dim3 grd((L.nx + 1 + FUSED_TX - 3) / (FUSED_TX - 2), (L.ny + 1 + FUSED_TY - 3) / (FUSED_TY - 2), (L.nz + 1 + lz - 1) / lz);
-    if (H->kernel == 0) {
+    if (kernel == 0) {
         DrTmaps T;
         const int c = H->cur;
         T.m[0] = H->tm_state[c][F_VX]; T.m[1] = H->tm_state[c][F_VY]; T.m[2] = H->tm_state[c][F_VZ]; T.m[3] = H->tm_G;
@@ -377,6 +495,15 @@ static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
     return DR_OK;
 }
 
+// DR_KERNEL 3: iterations `it` and `it + 1` (1-based) go into ONE sweep when both fit below `last_allowed` and `it` is not
+// itself a residual-check iteration (the sweep reports the residual of its second iteration only)
+static int sweep_len(const dr_handle* H, int it, int last_allowed, int ncheck) {
+    return (H->kernel == 3 && coded(H) && it + 1 <= last_allowed && (ncheck <= 0 || it % ncheck != 0)) ? 2 : 1;
+}
+static dr_status sweep(dr_handle* H, const DrPT& P, int n, bool with_res) {
+    return n == 2 ? iteration_coded(H, P, with_res, 2) : iteration(H, P, with_res);
+}
+
 // buffer whose stress slots hold the stresses: in the displacement form the sigma_aa slots of the state buffer carry
 // w, and the stresses (Hooke's law of the displacement BEFORE the last update, like the oracle's) sit in the other one
 static int stress_buf(const dr_handle* H) { return H->form ? H->cur ^ 1 : H->cur; }
@@ -395,20 +522,26 @@ static dr_status ensure_stresses(dr_handle* H) {
 }
 
 static dr_status read_residual(dr_handle* H, double* r) {
-    CK(cudaMemcpyAsync(H->pinned, H->res_bits, 8, cudaMemcpyDeviceToHost, H->st));
+    CK(cudaMemcpyAsync(H->pinned + 8, H->res_bits, 8, cudaMemcpyDeviceToHost, H->st));
     CK(cudaStreamSynchronize(H->st));
-    std::memcpy(r, H->pinned, 8);
+    std::memcpy(r, H->pinned + 8, 8);
     return DR_OK;
 }
 
-static dr_status averages(dr_handle* H, int lc, double eps0) {
+// enqueue the volume averages (Eq. 7) and their copy into pinned[dst .. dst+5]; no synchronisation
+static dr_status enqueue_averages(dr_handle* H, int dst) {
     const DrLayout& L = H->L;
     { dr_status es = ensure_stresses(H); if (es != DR_OK) return es; }
     k_avg_partial<<<DR_AVG_BLOCKS, DR_AVG_THREADS, 0, H->st>>>(H->L, cfields_of(H, stress_buf(H)), H->partial);
     CKL("k_avg_partial");
     k_avg_final<<<1, 256, 0, H->st>>>(H->partial, DR_AVG_BLOCKS, 1.0 / ((double)L.nx * L.ny * L.nz), H->avg_dev);
     CKL("k_avg_final");
-    CK(cudaMemcpyAsync(H->pinned, H->avg_dev, 6 * sizeof(double), cudaMemcpyDeviceToHost, H->st));
+    CK(cudaMemcpyAsync(H->pinned + dst, H->avg_dev, 6 * sizeof(double), cudaMemcpyDeviceToHost, H->st));
+    return DR_OK;
+}
+
+static dr_status averages(dr_handle* H, int lc, double eps0) {
+    { dr_status es = enqueue_averages(H, 0); if (es != DR_OK) return es; }
     CK(cudaEventRecord(H->e1, H->st));
     CK(cudaStreamSynchronize(H->st));
     for (int m = 0; m < 6; ++m) { H->avg[m] = H->pinned[m]; H->Ccol[lc][m] = H->avg[m] / eps0; }   // Eq. 9, 22
@@ -419,6 +552,22 @@ static dr_status averages(dr_handle* H, int lc, double eps0) {
     return DR_OK;
 }
 
+// second stopping rule (Reading R9b): state of the <sigma> stagnation test of one solve
+struct DrStag {
+    bool have_prev = false;
+    double prev[6] = {0, 0, 0, 0, 0, 0};
+    int calm = 0;
+    // a[6] = <sigma> at this check; true when two consecutive checks moved <sigma> by <= stag_tol (relative, max-norm)
+    bool update(const double* a, double stag_tol) {
+        double num = 0.0, den = 0.0;
+        for (int m = 0; m < 6; ++m) { num = std::max(num, std::fabs(a[m] - prev[m])); den = std::max(den, std::fabs(a[m])); }
+        if (have_prev && num <= stag_tol * den) ++calm; else calm = 0;
+        for (int m = 0; m < 6; ++m) prev[m] = a[m];
+        have_prev = true;
+        return calm >= 2;
+    }
+};
+
 static bool bad_lc(dr_handle* H, int lc, double eps0) {
     if (lc < 0 || lc > 5 || !(eps0 != 0.0) || !std::isfinite(eps0)) { H->err = "bad load case or eps0"; return true; }
     return false;
@@ -426,6 +575,7 @@ static bool bad_lc(dr_handle* H, int lc, double eps0) {
 
 extern "C" dr_status dr_solve(dr_handle* H, int lc, double eps0, double tol, int maxiter) {
     if (!H) return DR_ERR_ARG;
+    DrDeviceGuard dg(H->device);
     if (bad_lc(H, lc, eps0)) return DR_ERR_ARG;
     if (!(tol > 0.0) || maxiter < 1) return fail(H, DR_ERR_ARG, "bad tol or maxiter");
     CK(cudaEventRecord(H->e0, H->st));
@@ -434,19 +584,27 @@ extern "C" dr_status dr_solve(dr_handle* H, int lc, double eps0, double tol, int
     const DrPT P = make_pt(H, lc, eps0);
     dr_status status = DR_MAXITER;
     H->residual = INFINITY;
+    H->stop_reason = DR_STOP_MAXITER;
+    DrStag stag;
+    const bool use_stag = H->stag_tol > 0.0;
     int it;
     for (it = 1; it <= maxiter; ++it) {
+        const int n = sweep_len(H, it, maxiter, H->ncheck);
+        it += n - 1;                                          // index of the last iteration of this sweep
         const bool chk = (it % H->ncheck == 0);
         if (chk) CK(cudaMemsetAsync(H->res_bits, 0, 8, H->st));
-        s = iteration(H, P, chk);
+        s = sweep(H, P, n, chk);
         if (s != DR_OK) return s;
         if (chk) {
+            // the averages of the stagnation rule ride on the same synchronisation as the residual
+            if (use_stag) { s = enqueue_averages(H, 9); if (s != DR_OK) return s; }
             double r;
             s = read_residual(H, &r);
             if (s != DR_OK) return s;
             H->residual = r;
-            if (!std::isfinite(r)) { status = DR_ERR_DIVERGED; break; }
-            if (r <= tol) { status = DR_OK; break; }
+            if (!std::isfinite(r)) { status = DR_ERR_DIVERGED; H->stop_reason = DR_STOP_NONE; break; }
+            if (r <= tol) { status = DR_OK; H->stop_reason = DR_STOP_RESIDUAL; break; }
+            if (use_stag && stag.update(H->pinned + 9, H->stag_tol)) { status = DR_OK; H->stop_reason = DR_STOP_STAGNATION; break; }
         }
     }
     H->iters = std::min(it, maxiter);
@@ -476,8 +634,11 @@ extern "C" dr_status dr_solve_six(dr_handle* const h[6], double eps0, double tol
     int it[6];
     bool active[6], pending[6];
     dr_status st[6];
+    DrStag stag[6];
     for (int lc = 0; lc < 6; ++lc) {
         dr_handle* H = h[lc];
+        DrDeviceGuard dg(H->device);
+        H->stop_reason = DR_STOP_MAXITER;
         CK(cudaEventRecord(H->e0, H->st));
         dr_status s = prepare(H, lc, eps0);
         if (s != DR_OK) return s;
@@ -488,29 +649,36 @@ extern "C" dr_status dr_solve_six(dr_handle* const h[6], double eps0, double tol
         for (int lc = 0; lc < 6; ++lc) {
             if (!active[lc]) continue;
             dr_handle* H = h[lc];
-            const int n = std::min(H->ncheck - it[lc] % H->ncheck, maxiter - it[lc]);
+            DrDeviceGuard dg(H->device);
+            const int upto = it[lc] + std::min(H->ncheck - it[lc] % H->ncheck, maxiter - it[lc]);   // next check, or maxiter
             bool chk = false;
-            for (int i = 0; i < n; ++i) {
-                ++it[lc];
+            while (it[lc] < upto) {
+                const int n = sweep_len(H, it[lc] + 1, upto, H->ncheck);
+                it[lc] += n;
                 chk = (it[lc] % H->ncheck == 0);
                 if (chk) CK(cudaMemsetAsync(H->res_bits, 0, 8, H->st));
-                dr_status s = iteration(H, P[lc], chk);
+                dr_status s = sweep(H, P[lc], n, chk);
                 if (s != DR_OK) return s;
             }
-            if (chk) CK(cudaMemcpyAsync(H->pinned, H->res_bits, 8, cudaMemcpyDeviceToHost, H->st));
+            if (chk) {
+                if (H->stag_tol > 0.0) { dr_status s = enqueue_averages(H, 9); if (s != DR_OK) return s; }
+                CK(cudaMemcpyAsync(H->pinned + 8, H->res_bits, 8, cudaMemcpyDeviceToHost, H->st));
+            }
             pending[lc] = chk;
         }
         any = false;
         for (int lc = 0; lc < 6; ++lc) {
             if (!active[lc]) continue;
             dr_handle* H = h[lc];
+            DrDeviceGuard dg(H->device);
             if (pending[lc]) {
                 CK(cudaStreamSynchronize(H->st));
                 double r;
-                std::memcpy(&r, H->pinned, 8);
+                std::memcpy(&r, H->pinned + 8, 8);
                 H->residual = r;
-                if (!std::isfinite(r)) { st[lc] = DR_ERR_DIVERGED; active[lc] = false; H->err = "residual is not finite"; }
-                else if (r <= tol) { st[lc] = DR_OK; active[lc] = false; }
+                if (!std::isfinite(r)) { st[lc] = DR_ERR_DIVERGED; active[lc] = false; H->stop_reason = DR_STOP_NONE; H->err = "residual is not finite"; }
+                else if (r <= tol) { st[lc] = DR_OK; active[lc] = false; H->stop_reason = DR_STOP_RESIDUAL; }
+                else if (H->stag_tol > 0.0 && stag[lc].update(H->pinned + 9, H->stag_tol)) { st[lc] = DR_OK; active[lc] = false; H->stop_reason = DR_STOP_STAGNATION; }
             }
             if (active[lc] && it[lc] >= maxiter) { active[lc] = false; H->err = "maxiter reached"; }
             any = any || active[lc];
@@ -519,6 +687,7 @@ extern "C" dr_status dr_solve_six(dr_handle* const h[6], double eps0, double tol
     dr_status worst = DR_OK;
     for (int lc = 0; lc < 6; ++lc) {
         dr_handle* H = h[lc];
+        DrDeviceGuard dg(H->device);
         H->iters = it[lc];
         if (st[lc] != DR_ERR_DIVERGED) { dr_status s = averages(H, lc, eps0); if (s != DR_OK) return s; }
         if (status_out) status_out[lc] = (int)st[lc];
@@ -541,6 +710,7 @@ extern "C" dr_status dr_effective_C_six(dr_handle* const h[6], double out[36]) {
 
 extern "C" dr_status dr_step(dr_handle* H, int lc, double eps0, int niter) {
     if (!H) return DR_ERR_ARG;
+    DrDeviceGuard dg(H->device);
     if (bad_lc(H, lc, eps0)) return DR_ERR_ARG;
     if (niter < 0) return fail(H, DR_ERR_ARG, "bad niter");
     CK(cudaEventRecord(H->e0, H->st));
@@ -549,9 +719,11 @@ extern "C" dr_status dr_step(dr_handle* H, int lc, double eps0, int niter) {
     const DrPT P = make_pt(H, lc, eps0);
     double r = 0.0;
     for (int it = 1; it <= niter; ++it) {
+        const int n = sweep_len(H, it, niter, 0);
+        it += n - 1;
         const bool last = (it == niter);
         if (last) CK(cudaMemsetAsync(H->res_bits, 0, 8, H->st));
-        s = iteration(H, P, last);
+        s = sweep(H, P, n, last);
         if (s != DR_OK) return s;
     }
     if (niter > 0) { s = read_residual(H, &r); if (s != DR_OK) return s; }
@@ -561,13 +733,16 @@ extern "C" dr_status dr_step(dr_handle* H, int lc, double eps0, int niter) {
 
 extern "C" dr_status dr_iterate(dr_handle* H, int lc, double eps0, int niter) {
     if (!H) return DR_ERR_ARG;
+    DrDeviceGuard dg(H->device);
     if (bad_lc(H, lc, eps0)) return DR_ERR_ARG;
     if (niter < 0) return fail(H, DR_ERR_ARG, "bad niter");
     if (!H->have_fields || lc != H->cur_lc || eps0 != H->cur_eps0)
         return fail(H, DR_ERR_STATE, "dr_iterate needs a previous dr_step/dr_solve with the same load case and eps0");
     const DrPT P = make_pt(H, lc, eps0);
-    for (int it = 0; it < niter; ++it) {
-        dr_status s = iteration(H, P, false);
+    for (int it = 1; it <= niter; ++it) {
+        const int n = sweep_len(H, it, niter, 0);
+        it += n - 1;
+        dr_status s = sweep(H, P, n, false);
         if (s != DR_OK) return s;
     }
     return DR_OK;
@@ -597,6 +772,7 @@ extern "C" dr_status dr_info(dr_handle* H, int* iters, double* residual, double*
 
 extern "C" dr_status dr_get_field(dr_handle* H, int field, double* dst, size_t n) {
     if (!H || !dst) return DR_ERR_ARG;
+    DrDeviceGuard dg(H->device);
     if (field < 0 || field >= F_COUNT) return fail(H, DR_ERR_ARG, "bad field id");
     if (!H->have_fields) return fail(H, DR_ERR_STATE, "no fields yet");
     const DrLayout& L = H->L;
@@ -670,14 +846,21 @@ extern "C" dr_status dr_contribution_tensor(const double C_eff[36], const double
     return DR_OK;
 }
 
-extern "C" int dr_uses_palette(dr_handle* H) { return (H && H->has_pal && H->use_pal && H->kernel == 0) ? 1 : 0; }
+extern "C" int dr_uses_palette(dr_handle* H) { return (H && H->has_pal && H->use_pal && (H->kernel == 0 || H->kernel >= 3)) ? 1 : 0; }
+
+// kernel that the iterations of the last dr_step / dr_solve really ran: DR_KERNEL, except that 3 and 4 report 0 when the
+// image could not be stencil-coded (more than 256 distinct cell pairs, edge moduli or node stiffnesses)
+extern "C" int dr_active_kernel(dr_handle* H) { return !H ? -1 : (H->kernel >= 3 && !coded(H) ? 0 : H->kernel); }
 
 extern "C" long long dr_launch_count(dr_handle* H) { return H ? H->launches : 0; }
 
 extern "C" const char* dr_last_error(dr_handle* H) { return H ? H->err.c_str() : "null handle"; }
 
+extern "C" int dr_stop_reason(dr_handle* H) { return H ? H->stop_reason : (int)DR_STOP_NONE; }
+
 extern "C" void dr_destroy(dr_handle* H) {
     if (!H) return;
+    DrDeviceGuard dg(H->device);
     cudaStreamSynchronize(H->st);
     if (H->pinned) cudaFreeHost(H->pinned);
     if (H->e0) cudaEventDestroy(H->e0);

@@ -28,7 +28,9 @@ __global__ void k_pad_moduli(DrLayout L, const double* __restrict__ Ksrc, const 
     if (i > L.nx || j > L.ny) return;
     int ci = min(max(i, 0), L.nx - 1), cj = min(max(j, 0), L.ny - 1), ck = min(max(k, 0), L.nz - 1);
     size_t s = (size_t)ci + (size_t)L.nx * ((size_t)cj + (size_t)L.ny * ck);
-    double Kv = Ksrc[s], Gv = Gsrc[s];
+    // + 0.0 turns a -0.0 modulus into +0.0 (it passes the >= 0 test below): 1/(-0) = -inf next to a +0 cell would make
+    // the edge mean inf - inf = NaN, and its bit pattern would win the unsigned max of hmax
+    double Kv = Ksrc[s] + 0.0, Gv = Gsrc[s] + 0.0;
     long long q = L.origin + i + L.sy * j + L.sz * k;
     Kp[q] = Kv; Gp[q] = Gv;
     if (i == ci && j == cj && k == ck) {
@@ -243,9 +245,10 @@ __global__ void k_pal_build(long long N, const double* __restrict__ Ksrc, const 
                             unsigned long long* kK, unsigned long long* kG, unsigned int* flags) {
     const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= N || (*((volatile unsigned int*)flags) & 2u)) return;
-    const unsigned long long kb = (unsigned long long)__double_as_longlong(Ksrc[q]), gb = (unsigned long long)__double_as_longlong(Gsrc[q]);
+    // + 0.0: -0.0 and +0.0 are the same modulus (see k_pad_moduli)
+    const unsigned long long kb = (unsigned long long)__double_as_longlong(Ksrc[q] + 0.0), gb = (unsigned long long)__double_as_longlong(Gsrc[q] + 0.0);
     if (q > 0 && (threadIdx.x & 31) != 0) {          // same pair as the previous cell of the warp: that lane inserts it
-        if ((unsigned long long)__double_as_longlong(Ksrc[q - 1]) == kb && (unsigned long long)__double_as_longlong(Gsrc[q - 1]) == gb) return;
+        if ((unsigned long long)__double_as_longlong(Ksrc[q - 1] + 0.0) == kb && (unsigned long long)__double_as_longlong(Gsrc[q - 1] + 0.0) == gb) return;
     }
     if (dr_pal_insert(kK, kG, kb, gb) < 0) atomicOr(flags, 2u);
 }
@@ -262,7 +265,7 @@ __global__ void k_pal_assign(DrLayout L, const double* __restrict__ Ksrc, const 
     const int k = (int)blockIdx.z - 1;
     const int ci = min(max(i, 0), L.nx - 1), cj = min(max(j, 0), L.ny - 1), ck = min(max(k, 0), L.nz - 1);
     const size_t s = (size_t)ci + (size_t)L.nx * ((size_t)cj + (size_t)L.ny * ck);
-    const int slot = dr_pal_find(kK, kG, (unsigned long long)__double_as_longlong(Ksrc[s]), (unsigned long long)__double_as_longlong(Gsrc[s]));
+    const int slot = dr_pal_find(kK, kG, (unsigned long long)__double_as_longlong(Ksrc[s] + 0.0), (unsigned long long)__double_as_longlong(Gsrc[s] + 0.0));
     if (slot < 0) { atomicOr(flags, 4u); return; }
     const size_t blk = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
     ids[blk * (size_t)(TX * TY) + threadIdx.y * TX + threadIdx.x] = (unsigned char)slot;

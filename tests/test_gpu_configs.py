@@ -1,0 +1,179 @@
+"""GPU parity on the BASELINE.json configs themselves (SURVEY 8(d) "Runs per config"; north_star: "match the CPU oracle
+... on every config").  libdr through the C ABI against the CPU oracle on the same seeded images, at full size and in
+the default launch configuration (what bench.py times).
+
+Parity (i) fields: dr_step vs dro_step, 100 iterations at 191^3 (cfg 2, 3: all six load cases), 20 iterations at 479^3
+and 703^3 (cfg 4, 5: lc 2 and 4); per-field relative L-inf <= 1e-10.
+Parity (ii) converged C: cfg 2 (lc 2, 4) and cfg 3 with DR_VOID_REL 1e-5 (lc 0, 3) to tol 1e-8 with the same ncheck on both
+sides: same stopping iteration, |C_gpu - C_cpu| <= 1e-6 max|C|."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2410_20441_b200 import inputs
+from tests.test_gpu_parity import FIELD_TOL, C_TOL, field_errors, run_pair, to_dev, gpu, _host_gb  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+def exact_averages(o):
+    """<sigma> (Eq. 7, trapezoid weights of reading R7) from the oracle's exported FIELDS, summed in extended
+    precision (np.longdouble, pairwise) -- and, for the largest component, exactly (math.fsum of per-plane fsums).
+    This is the definition written out a third time, independent of the oracle's sequential loop and of k_avg_*."""
+    out = np.zeros(6)
+    N = None
+    big = None
+    for m, f in enumerate((3, 4, 5, 6, 7, 8)):
+        a = o.get_field(f)
+        if m < 3:
+            N = a.size
+            w = a
+        else:
+            w = a.copy()
+            # tyz (nz+1, ny+1, nx): weights 1/2 on the first/last j and k; txz: i and k; txy: i and j
+            ax = {3: (0, 1), 4: (0, 2), 5: (1, 2)}[m]
+            for d in ax:
+                sl = [slice(None)] * 3
+                sl[d] = 0; w[tuple(sl)] *= 0.5
+                sl[d] = -1; w[tuple(sl)] *= 0.5
+        out[m] = float(np.sum(w, dtype=np.longdouble) / N)
+        if big is None or abs(out[m]) > abs(big[1]):
+            big = (m, out[m], w)
+        else:
+            del w
+    m, _, w = big
+    exact = math.fsum(math.fsum(plane.ravel().tolist()) for plane in w) / N
+    return out, m, exact
+
+
+# ------------------------------------------------------------------------------------------------ cfg 2 (191^3, fluid spheroid)
+def test_cfg2_fields_100_iterations_all_load_cases(oracle_mod, gpu):
+    K, G, _ = inputs.config2_spheroid()
+    for lc in range(6):
+        errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, 1e-4, 100)
+        assert max(errs) <= FIELD_TOL, (lc, errs)
+        assert abs(ro - rs) <= 1e-9 * ro
+        assert np.max(np.abs(ao - as_)) <= 1e-10 * np.max(np.abs(ao)), lc
+
+
+def test_cfg2_converged_C_vs_oracle_and_contribution_tensor(oracle_mod, gpu):
+    """cfg 2 to tol 1e-8: lc 2 and lc 4 against the oracle (same ncheck -> same stopping iteration, column within
+    1e-6 max|C|); then the whole C on the GPU, its exact symmetries (tetragonal about z), and dr_contribution_tensor
+    (Eq. 23) against oracle/post.py on that tensor and the matrix-only run."""
+    from oracle import post
+    K, G, m = inputs.config2_spheroid()
+    s = gpu.Solver(to_dev(K), to_dev(G), ncheck=100)
+    C, log = s.solve_all(1e-4, 1e-8, 19100)
+    assert all(l[0] == 0 for l in log), log
+    assert s.stop_reason() == gpu.STOP_RESIDUAL
+    o = oracle_mod.Oracle(K, G, ncheck=100)
+    for lc in (2, 4):
+        assert o.solve(lc, 1e-4, 1e-8, 19100) == 0
+        it, r, _ = o.info()
+        assert it == log[lc][1], (lc, it, log[lc][1])
+        assert abs(r - log[lc][2]) <= 1e-6 * r
+        col = o.avg_stress() / 1e-4
+        assert np.max(np.abs(col - C[:, lc])) <= C_TOL * np.max(np.abs(C)), (lc, col, C[:, lc])
+    s0 = C[0, 0]
+    assert abs(C[0, 0] - C[1, 1]) <= 1e-9 * s0 and abs(C[0, 2] - C[1, 2]) <= 1e-9 * s0 and abs(C[3, 3] - C[4, 4]) <= 1e-9 * s0
+    assert C[2, 2] < C[0, 0] and C[3, 3] < C[5, 5]          # softest across the thin (z) direction of the oblate inclusion
+    s.close()
+    # matrix-only run = Hooke (pin P1), solved on the GPU as the config asks
+    K1, G1 = inputs.homogeneous(191, 70.2, 29.0)
+    s1 = gpu.Solver(to_dev(K1), to_dev(G1), ncheck=100)
+    C1, log1 = s1.solve_all(1e-4, 1e-8, 19100)
+    assert all(l[0] == 0 and l[1] == 100 for l in log1)
+    phi = float(m.mean())
+    H = gpu.contribution_tensor(C, C1, phi)
+    Ho = post.contribution_tensor(C, C1, phi)
+    assert np.max(np.abs(H - Ho)) <= 1e-9 * np.max(np.abs(Ho))
+    assert all(H[a, a] > 0 for a in range(6))
+    assert abs(H[0, 0] - H[1, 1]) <= 1e-6 * H[2, 2] and abs(H[3, 3] - H[4, 4]) <= 1e-6 * H[3, 3]
+
+
+# ------------------------------------------------------------------------------------------------ cfg 3 (191^3, 200 pores, 1e-6)
+def test_cfg3_fields_100_iterations_all_load_cases(oracle_mod, gpu):
+    K, G, _ = inputs.config3_random_spheres()
+    for lc in range(6):
+        errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, 1e-4, 100)
+        assert max(errs) <= FIELD_TOL, (lc, errs)
+        assert abs(ro - rs) <= 1e-9 * ro
+        assert np.max(np.abs(ao - as_)) <= 1e-10 * np.max(np.abs(ao)), lc
+
+
+def test_cfg3_converged_C_with_void_clamp_vs_oracle(oracle_mod, gpu):
+    """cfg 3 with DR_VOID_REL = 1e-5 (reading R9: as given the max-norm plateaus), lc 0 and lc 3, tol 1e-8"""
+    K, G, _ = inputs.config3_random_spheres()
+    s = gpu.Solver(to_dev(K), to_dev(G), ncheck=100, void_rel=1e-5)
+    o = oracle_mod.Oracle(K, G, ncheck=100, void_rel=1e-5)
+    for lc in (0, 3):
+        assert s.solve(lc, 1e-4, 1e-8, 19100) == 0 and s.stop_reason() == gpu.STOP_RESIDUAL
+        assert o.solve(lc, 1e-4, 1e-8, 19100) == 0 and o.stop_reason() == oracle_mod.STOP_RESIDUAL
+        assert s.info()[0] == o.info()[0], (lc, s.info(), o.info())
+        cs, co = s.avg_stress() / 1e-4, o.avg_stress() / 1e-4
+        assert np.max(np.abs(cs - co)) <= C_TOL * np.max(np.abs(co)), (lc, cs, co)
+
+
+def test_cfg3_as_given_stops_on_stagnation_like_the_oracle(oracle_mod, gpu):
+    """cfg 3 as given (contrast 1e-6, no clamp): the residual plateaus near 2e-5; the stagnation rule (reading R9b) ends
+    the solve with DR_OK on both sides at the same check, with the same column."""
+    K, G, _ = inputs.config3_random_spheres()
+    s = gpu.Solver(to_dev(K), to_dev(G), ncheck=100)
+    o = oracle_mod.Oracle(K, G, ncheck=100)
+    lc = 3
+    assert s.solve(lc, 1e-4, 1e-8, 19100) == 0
+    assert o.solve(lc, 1e-4, 1e-8, 19100) == 0
+    assert s.stop_reason() == gpu.STOP_STAGNATION and o.stop_reason() == oracle_mod.STOP_STAGNATION
+    assert s.info()[0] < 19100 and s.info()[1] > 1e-8
+    # the decision compares a 1e-10 change of <sigma>; the two sums differ at 1e-12: allow the stop one check apart
+    assert abs(s.info()[0] - o.info()[0]) <= 100, (s.info(), o.info())
+    cs, co = s.avg_stress() / 1e-4, o.avg_stress() / 1e-4
+    assert np.max(np.abs(cs - co)) <= C_TOL * np.max(np.abs(co))
+
+
+# ------------------------------------------------------------------------------------------------ cfg 4 (479^3), cfg 5 (703^3)
+def test_cfg4_479_fields_20_iterations_and_which_side_carries_the_average_error(oracle_mod, gpu):
+    """cfg 4 at full size, lc 2 and lc 4, 20 iterations.  Averages: round 1 loosened the bar to 1e-9 at this
+    size arguing that the ORACLE's sequential sum of 1.1e8 terms carries the difference.  Measured here: <sigma> from the
+    oracle's own fields in extended precision and exactly (fsum) -- the GPU's pairwise two-pass sum must agree with
+    THAT to 1e-12, the oracle's sequential sum is allowed its N-term rounding error."""
+    if _host_gb() < 40:
+        pytest.skip("oracle needs ~16 GB of host memory at 479^3")
+    K, G, _ = inputs.config4_grf()
+    for lc in (2, 4):
+        o = oracle_mod.Oracle(K, G)
+        s = gpu.Solver(to_dev(K), to_dev(G))
+        o.step(lc, 1e-4, 20)
+        s.step(lc, 1e-4, 20)
+        errs = field_errors(o, s, K, G, 1e-4)
+        assert max(errs) <= FIELD_TOL, (lc, errs)
+        assert abs(o.info()[1] - s.info()[1]) <= 1e-9 * o.info()[1]
+        ext, m, exact = exact_averages(o)
+        scale = np.max(np.abs(ext))
+        assert abs(ext[m] - exact) <= 1e-15 * scale                      # longdouble pairwise = exact sum here
+        gpu_err = np.max(np.abs(s.avg_stress() - ext)) / scale
+        ora_err = np.max(np.abs(o.avg_stress() - ext)) / scale
+        print("cfg4 lc %d: <sigma> error vs exact sum: GPU %.2e, oracle (sequential) %.2e" % (lc, gpu_err, ora_err))
+        assert gpu_err <= 1e-12, (lc, gpu_err, ora_err)
+        assert ora_err <= 1e-9, (lc, ora_err)
+        s.close(); del s, o
+
+
+def test_cfg5_703_fields_20_iterations(oracle_mod, gpu):
+    """cfg 5 at full size (703^3, the largest), lc 2 and lc 4, 20 iterations"""
+    import torch
+    if _host_gb() < 90:
+        pytest.skip("oracle needs ~45 GB of host memory at 703^3")
+    K, G, _ = inputs.config5_penny_cracks()
+    Kd, Gd = to_dev(K), to_dev(G)
+    for lc in (2, 4):
+        o = oracle_mod.Oracle(K, G)
+        s = gpu.Solver(Kd, Gd)
+        o.step(lc, 1e-4, 20)
+        s.step(lc, 1e-4, 20)
+        errs = field_errors(o, s, K, G, 1e-4)
+        assert max(errs) <= FIELD_TOL, (lc, errs)
+        assert abs(o.info()[1] - s.info()[1]) <= 1e-9 * o.info()[1]
+        s.close(); del s, o
+        torch.cuda.empty_cache()

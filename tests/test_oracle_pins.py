@@ -446,6 +446,31 @@ def test_void_clamp_equals_zeroing_that_phase_by_hand(oracle_mod):
     assert np.array_equal(d.get_field(0), c.get_field(0))
 
 
+def test_stagnation_rule_stops_on_the_fixed_point_when_the_residual_plateaus(oracle_mod):
+    """Reading R9b: a stiff grain floating in a 1e-6-contrast pore is held by pore-stiffness springs only; the max-norm
+    residual plateaus near 1e-6 for ever (DRO_MAXITER without the rule).  With the rule the solve stops with DRO_OK and
+    stop_reason = STAGNATION, and the C it reports is the fixed point of the discrete problem: equal to the dense
+    brute-force solve to 1e-8 -- i.e. the rule does not stop early."""
+    K = np.full((6, 6, 6), 37.0); G = np.full((6, 6, 6), 44.0)
+    K[1:4, 2:5, 1:4] = 37e-6; G[1:4, 2:5, 1:4] = 44e-6
+    K[2, 3, 2] = 37.0; G[2, 3, 2] = 44.0
+    Cb = bruteforce.effective_C(K, G, 1e-4, 1.0, 0)
+    o = oracle_mod.Oracle(K, G, ncheck=20)
+    C, log = o.solve_all(1e-4, 1e-8, 6000)
+    assert all(st == 0 and it < 1000 and r > 1e-8 for st, it, r in log), log
+    assert o.stop_reason() == oracle_mod.STOP_STAGNATION
+    assert np.max(np.abs(C - Cb)) <= 1e-8 * np.max(Cb)
+    # rule off: the same solve runs into maxiter (soft status) with the same C
+    o2 = oracle_mod.Oracle(K, G, ncheck=20, stag_tol=0.0)
+    assert o2.solve(2, 1e-4, 1e-8, 1500) == oracle_mod.MAXITER and o2.stop_reason() == oracle_mod.STOP_MAXITER
+    assert np.max(np.abs(o2.avg_stress() / 1e-4 - Cb[:, 2])) <= 1e-8 * np.max(Cb)
+    # where the residual does reach tol the rule never fires first (same iteration counts as the survey probe: P14)
+    Kh, Gh, _ = inputs.config1_sphere(n=16, r=3.0)
+    a = oracle_mod.Oracle(Kh, Gh); b = oracle_mod.Oracle(Kh, Gh, stag_tol=0.0)
+    assert a.solve(1, 1e-4, 1e-8, 5000) == 0 and b.solve(1, 1e-4, 1e-8, 5000) == 0
+    assert a.info()[0] == b.info()[0] and a.stop_reason() == oracle_mod.STOP_RESIDUAL
+
+
 # ---------------------------------------------------------------- ABI behaviour
 def test_argument_checks(oracle_mod):
     K, G = inputs.homogeneous(3)
