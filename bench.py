@@ -9,7 +9,7 @@ A "step" is one PT iteration of the whole hot path as dr_solve runs it: the fuse
 the initial/boundary fields (a4) and the volume averages -> C column (a6).  The timed region is ONE
 dr_solve(lc, eps0, tol=1e-300, maxiter=K) call, i.e. exactly K steps.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg2|cfg1|cfg5] [--time-to-solution]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg2|cfg1|cfg5] [--kernel 3|0|1|2|4] [--time-to-solution]
     python bench.py --impl reference ...      # the CPU oracle on the host cores (bounded sample)
 
 N > 1 (torchrun): the path shards over independent load cases -- rank r solves load case r mod 6 of the same
@@ -31,11 +31,33 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 from paper_2410_20441_b200 import inputs, shard  # noqa: E402
+from paper_2410_20441_b200 import build as drbuild  # noqa: E402
 
 BYTES_PER_VOXEL_ITER = 160.0        # (2*9 + 2) fp64, SURVEY 8(d)
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of k_pt_tma at 479^3 from the one `ncu --set full` capture
-# summarised in profiles/r1_summary.md (8.96 + 7.95 GB with the phase ids, 10.96 + 7.99 GB with fp64 K, G); null for any other workload / kernel
-NCU_TRAFFIC_BYTES = {("cfg4", 0, 1): 16.91e9, ("cfg4", 0, 0): 18.94e9}      # (workload, kernel, palette)
+KERNEL_NAMES = {0: "k_pt_tma", 1: "k_stress_split+k_velocity_split", 2: "k_pt_fused", 3: "k_pt_tb2<.,2> (two iterations per sweep)",
+                4: "k_pt_tb2<.,1>"}
+KERNEL_DESC = {0: "fused+TMA", 1: "split", 2: "fused+LDG", 3: "fused+TMA, stencil codes, 2 iterations per sweep", 4: "fused+TMA, stencil codes"}
+
+
+def ncu_traffic(workload, kernel, palette, form):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the `ncu --set full` captures
+    listed in profiles/traffic.csv -- only a row taken with the CURRENT kernel sources (build.source_hash) counts; a capture of
+    older kernels says nothing about this binary, so the answer is then null."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        cur = drbuild.source_hash()
+        with open(path) as fh:
+            for line in fh:
+                t = [x.strip() for x in line.split(",")]
+                if len(t) < 8 or t[0].startswith("#") or t[0] == "source_hash":
+                    continue
+                if t[0] == cur and t[1] == workload and int(t[2]) == kernel and int(t[3]) == palette and int(t[4]) == form:
+                    return float(t[5]) + float(t[6])
+    except Exception:
+        pass
+    return None
+
+
 WORKLOADS = {
     "cfg1": dict(n=32, gen="config1_sphere", desc="32^3 centred spherical pore r=5, contrast 1e-6"),
     "cfg2": dict(n=191, gen="config2_spheroid", desc="191^3 oblate fluid spheroid (40,40,8)"),
@@ -178,7 +200,8 @@ def main():
     ap.add_argument("--lc", type=int, default=2)
     ap.add_argument("--eps0", type=float, default=1e-4)
     ap.add_argument("--ncheck", type=int, default=100)
-    ap.add_argument("--kernel", type=int, default=0, help="0 fused with TMA staging (default), 1 split baseline, 2 fused with LDG prefetch")
+    ap.add_argument("--kernel", type=int, default=3, help="3 two PT iterations per sweep on stencil-coded images (default; falls back to 0), 0 fused with TMA staging, 1 split baseline, 2 fused with LDG prefetch, 4 coded one-iteration sweep")
+    ap.add_argument("--sustained-seconds", type=float, default=3.0, help="length of the back-to-back dr_iterate run behind the `sustained` block (0 = skip)")
     ap.add_argument("--form", type=int, default=0, help="0 stress-relaxation form of the paper (default, 160 B/voxel), 1 displacement form (112 B/voxel)")
     ap.add_argument("--palette", type=int, default=1, help="1 (default): uint8 phase ids + table when the image has <= 256 distinct (K,G); 0: fp64 modulus fields")
     ap.add_argument("--cpu-sample-n", type=int, default=191)
@@ -216,7 +239,8 @@ def main():
     lc = shard.load_case_of_rank(rank, world, args.lc)
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
-        s = binding.Solver(Kd, Gd, stream=stream, ncheck=args.ncheck, kernel=args.kernel, form=args.form, palette=args.palette)
+        # stag_tol 0: the timed dr_solve must run exactly K steps (the stagnation rule could end it early)
+        s = binding.Solver(Kd, Gd, stream=stream, ncheck=args.ncheck, kernel=args.kernel, form=args.form, palette=args.palette, stag_tol=0.0)
 
         def barrier():
             torch.cuda.synchronize(dev)
@@ -248,8 +272,24 @@ def main():
         torch.cuda.synchronize(dev)
         kms = k0.elapsed_time(k1) / args.steps
         clocks = sampler.stop() if rank == 0 else None
+        active_kernel = s.active_kernel()
+        # ---- sustained: what a real solve gets.  >= 3 s of back-to-back PT iterations (no residual check, no host sync) with
+        # its own clock record: under the 1 kW cap the SM clock settles below what a 0.1 s burst sees.
+        sustained = None
+        if args.sustained_seconds > 0 and rank == 0:
+            n_sus = max(2 * int(args.sustained_seconds / (kms * 1e-3) / 2 + 1), 2)
+            smp2 = ClockSampler(local)
+            smp2.start()
+            q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            q0.record(stream)
+            s.iterate(lc, args.eps0, n_sus)
+            q1.record(stream)
+            torch.cuda.synchronize(dev)
+            sus_ms = q0.elapsed_time(q1) / n_sus
+            sustained = {"iterations": n_sus, "seconds": sus_ms * n_sus * 1e-3, "ms_per_step": sus_ms, "clocks": smp2.stop()}
         if dist is not None:
             ms = shard.max_over_ranks(ms, dist, dev)
+            kms = shard.max_over_ranks(kms, dist, dev)
 
         # ---- e2e through the C-ABI call with HOST buffers (H2D of K,G and D2H of C inside the timed region)
         # every rank runs the call on its own GPU (N independent images: weak scaling); time = max over ranks
@@ -269,7 +309,7 @@ def main():
             nsteps = sum(iters)
             e2e = {"value": world * N * nsteps / dt, "unit": "voxel-updates/s",
                    "h2d_bytes_per_step": 2 * N * 8 / nsteps, "d2h_bytes_per_step": (36 * 8 + 6 * 8 * (args.e2e_iters // args.ncheck)) / nsteps,
-                   "call": "dr_solve_image_host: H2D K,G + dr_create + 6 load cases x %d iterations + C read back" % args.e2e_iters,
+                   "call": "dr_solve_image_host (library defaults, DR_KERNEL 3): H2D K,G + dr_create + 6 load cases x %d iterations + C read back" % args.e2e_iters,
                    "seconds": dt}
             del stage, Kh, Gh
             # the solver's workspace was reused by the e2e call: rebuild the handle state
@@ -296,24 +336,41 @@ def main():
     bpv = 112.0 if args.form == 1 else BYTES_PER_VOXEL_ITER      # algorithmic bytes per voxel-iteration of the form
     value = shard.job_throughput(N, args.steps, world, ms)
     teff = bpv * N * args.steps / (ms * 1e-3) / 1e9
-    kern_gbs = bpv * N / (kms * 1e-3) / 1e9
+    # one launch of the dominant kernel advances N voxels by `ipl` iterations: algorithmic bytes per launch = ipl x bpv x N
+    ipl = 2 if active_kernel == 3 else 1
+    launch_ms = kms * ipl
+    kern_gbs = ipl * bpv * N / (launch_ms * 1e-3) / 1e9
+    traffic = ncu_traffic(args.workload, active_kernel, int(pal_active), args.form) if args.n is None else None
+    roof = {"bound": "hbm", "kernel": KERNEL_NAMES[active_kernel], "achieved": kern_gbs, "peak": peak, "unit": "GB/s", "frac": kern_gbs / peak,
+            "traffic": traffic, "peak_source": peak_src, "launch_ms": launch_ms, "iterations_per_launch": ipl,
+            "algorithmic_bytes_per_launch": ipl * bpv * N,
+            "note": "achieved = ALGORITHMIC bytes (160 B per voxel-iteration, SURVEY 8(d)) / launch time: with two iterations per sweep it "
+                    "may exceed the DRAM rate; physical = ncu dram bytes / launch time"}
+    if traffic is not None:
+        roof["physical_GBs"] = traffic / (launch_ms * 1e-3) / 1e9
+        roof["physical_frac"] = roof["physical_GBs"] / peak
+        roof["traffic_source"] = "profiles/traffic.csv row for source hash %s" % drbuild.source_hash()
     line = {
         "metric": "pt_voxel_updates_per_s", "value": value, "unit": "voxel-updates/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s: %s" % (args.workload, WORKLOADS[args.workload]["desc"]), "grid": [n, n, n],
-                   "load_case": lc, "ncheck": args.ncheck, "form": "stress-relaxation (paper, 160 B/voxel-iteration)" if args.form == 0 else "displacement (112 B/voxel-iteration)", "kernel": {0: "fused+TMA", 1: "split", 2: "fused+LDG"}[args.kernel], "moduli": "uint8 phase ids + 256-entry table" if pal_active else "fp64 K, G fields",
+                   "load_case": lc, "ncheck": args.ncheck, "form": "stress-relaxation (paper, 160 B/voxel-iteration)" if args.form == 0 else "displacement (112 B/voxel-iteration)",
+                   "kernel": KERNEL_DESC[active_kernel], "kernel_requested": args.kernel,
+                   "moduli": "uint8 phase ids + 256-entry table" if pal_active else "fp64 K, G fields",
                    "parallelism": "load cases sharded over %d GPU(s), no collective" % world,
-                   "l2": "inputs (%.1f GB per iteration) larger than L2; no flush needed" % (BYTES_PER_VOXEL_ITER * N / 1e9)},
+                   "l2": "inputs (%.1f GB per sweep) larger than L2; no flush needed" % (BYTES_PER_VOXEL_ITER * N / 1e9)},
         "T_eff_GBs": teff, "T_eff_frac_of_measured_peak": teff / peak, "T_eff_frac_of_8000_nominal": teff / 8000.0,
         "clocks": clocks,
         "e2e": e2e,
         "gpu_launches": int(launches),
-        "roofline": {"bound": "hbm", "kernel": {0: "k_pt_tma", 1: "k_stress_split+k_velocity_split", 2: "k_pt_fused"}[args.kernel],
-                     "achieved": kern_gbs, "peak": peak, "unit": "GB/s", "frac": kern_gbs / peak,
-                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.kernel, int(pal_active))) if (args.n is None and args.form == 0) else None, "peak_source": peak_src, "launch_ms": kms,
-                     "algorithmic_bytes_per_launch": bpv * N},
+        "roofline": roof,
     }
+    if sustained is not None:
+        sus_gbs = bpv * N / (sustained["ms_per_step"] * 1e-3) / 1e9
+        sustained.update({"value": N / (sustained["ms_per_step"] * 1e-3), "unit": "voxel-updates/s", "T_eff_GBs": sus_gbs,
+                          "frac": sus_gbs / peak, "what": "back-to-back dr_iterate, same handle and load case, no host synchronisation"})
+        line["sustained"] = sustained
     if tts is not None:
         line["time_to_full_C"] = tts
     if not args.no_cpu_baseline:

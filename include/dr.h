@@ -58,12 +58,12 @@ typedef enum {
     DR_GAVG = 3,       /* shear modulus on edges: 0 harmonic mean of the 4 cells [default], 1 arithmetic (R4) */
     DR_VOID_REL = 4,   /* r>0: cells with K+4G/3 <= r*max(K+4G/3) become exact void K=G=0 [0 = off] (R9)      */
     DR_BC_MODE = 5,    /* 0 paper's mixed BCs [default]; 1 full kinematic uniform BC on all faces (R5)        */
-    DR_KERNEL = 6,     /* 0 fused z-march kernel with TMA staging [default]; 1 split stress/velocity kernels
+    DR_KERNEL = 6,     /* 0 fused z-march kernel with TMA staging; 1 split stress/velocity kernels
                           (baseline); 2 fused z-march kernel with register-prefetched LDG loads;
-                          3 temporal blocking: TWO PT iterations per sweep (the state is read and written once per two
+                          3 [default] temporal blocking: TWO PT iterations per sweep (the state is read and written once per two
                           iterations) on stencil-coded images -- images with <= 256 distinct (K,G) pairs, edge moduli
                           and node stiffnesses, i.e. segmented rock images; other images, odd leftovers and a check
-                          iteration that is the first of a pair run kernel 0 (dr_active_kernel tells); stress form only;
+                          iteration that is the first of a pair run kernel 0 (dr_active_kernel tells), and so does DR_FORM 1;
                           4 one iteration per sweep with the coded kernel (A/B reference of 3)                          */
     DR_ZCHUNK = 7,     /* z layers per CTA of the fused kernels; 0 = automatic [default] (tuning knob)            */
     DR_PALETTE = 9,    /* 1 [default]: images with <= 256 distinct (K,G) pairs run the fused kernel on a uint8 phase id
@@ -92,6 +92,10 @@ typedef enum {
 /* Bytes of device workspace dr_create needs for an nx*ny*nz grid (0 if the sizes are invalid). */
 size_t dr_workspace_bytes(int nx, int ny, int nz);
 
+/* Bytes of device workspace for a handle that can also run dr_solve_all: six state sets instead of one (0 if the sizes are
+ * invalid).  191^3: 7.4 GB, 479^3: 111 GB, 703^3 does not fit one B200 -- the batch is meant for small and medium grids. */
+size_t dr_workspace_bytes_six(int nx, int ny, int nz);
+
 /* Create a solver.  nx,ny,nz >= 2; h > 0.
  * K, G: DEVICE pointers, nx*ny*nz doubles each, x fastest, >= 0 and finite (K = G = 0 is void, G = 0 with K > 0
  * is a fluid; both allowed).  They are read (copied into the workspace with a replicate halo) and not kept.
@@ -114,6 +118,18 @@ dr_status dr_set_param(dr_handle* h, int id, double value);
  * (DR_STAG_TOL), at most maxiter iterations; then the
  * volume averages (Eq. 7) and column load_case of C* (Eq. 9, 22).  eps0 != 0, tol > 0, maxiter >= 1. */
 dr_status dr_solve(dr_handle* h, int load_case, double eps0, double tol, int maxiter);
+
+/* The six load cases of the image advanced together on ONE handle (one direct test per stiffness column; the
+ * tests share K and G): every launch of the two-iteration kernel carries all load cases that have not met a stopping rule
+ * yet, so a small grid fills the GPU and needs a sixth of the launches.  Needs a workspace of dr_workspace_bytes_six() bytes
+ * at dr_create (else DR_ERR_WORKSPACE).  Same iterates, checks, stopping rules and C* as six dr_solve calls (on images that
+ * cannot be stencil-coded, or with DR_KERNEL != 3 / DR_FORM 1, it simply runs those six calls).  status_out: HOST, 6 ints
+ * (dr_status per load case) or NULL.  Returns the worst status; afterwards dr_effective_C and dr_info_lc are valid
+ * (dr_get_field is not: call dr_step / dr_solve for fields). */
+dr_status dr_solve_all(dr_handle* h, double eps0, double tol, int maxiter, int status_out[6]);
+
+/* Iterations done, last residual and dr_stop value of load case lc (0..5) in the last dr_solve_all.  Pointers may be NULL. */
+dr_status dr_info_lc(dr_handle* h, int load_case, int* iters, double* residual, int* stop);
 
 /* The six load cases at once on six solvers (h[lc] solves load case lc; six distinct handles, each with its own
  * workspace and, to overlap on the device, its own stream).  One host thread enqueues every unfinished load case up
@@ -152,8 +168,8 @@ dr_status dr_get_field(dr_handle* h, int field, double* dst_device, size_t n);
 
 /* Whole 6x6 tensor from HOST arrays through the public API with host<->device copies inside: allocates
  * nothing on the device itself -- K_host/G_host (nx*ny*nz doubles, pinned or pageable) are staged through
- * stage_device (DEVICE, >= 2*nx*ny*nz doubles, caller-owned), then dr_create + 6 x dr_solve + dr_effective_C
- * run in `workspace`.  C_out: HOST, 36 doubles.  iters_out: HOST, 6 ints or NULL.  Returns the worst status. */
+ * stage_device (DEVICE, >= 2*nx*ny*nz doubles, caller-owned), then dr_create + the six load cases + dr_effective_C
+ * run in `workspace` (dr_solve_all if it has dr_workspace_bytes_six() bytes, else six dr_solve calls).  C_out: HOST, 36 doubles.  iters_out: HOST, 6 ints or NULL.  Returns the worst status. */
 dr_status dr_solve_image_host(int nx, int ny, int nz, double h,
                               const double* K_host, const double* G_host,
                               double* stage_device, void* workspace, size_t workspace_bytes, void* cuda_stream,

@@ -566,6 +566,29 @@ int dro_get_field(dro_handle* H, int field, double* dst, size_t n) {
     return DRO_OK;
 }
 
+/* raw state arrays for the z-slab halo test (tests/test_shard_gloo.py): 0 vx 1 vy 2 vz 3 p 4 txx 5 tyy 6 tzz 7 tyz 8 txz 9 txy,
+ * whole arrays, dense logical shape.  Pure copies: no arithmetic. */
+static std::vector<double>* raw_array(dro_handle* H, int id) {
+    switch (id) {
+        case 0: return &H->vx; case 1: return &H->vy; case 2: return &H->vz; case 3: return &H->p; case 4: return &H->txx;
+        case 5: return &H->tyy; case 6: return &H->tzz; case 7: return &H->tyz; case 8: return &H->txz; case 9: return &H->txy;
+    }
+    return nullptr;
+}
+size_t dro_raw_size(dro_handle* H, int id) { std::vector<double>* a = H ? raw_array(H, id) : nullptr; return a ? a->size() : 0; }
+int dro_get_raw(dro_handle* H, int id, double* dst, size_t n) {
+    std::vector<double>* a = H ? raw_array(H, id) : nullptr;
+    if (!a || !dst || n != a->size() || a->empty()) return DRO_ERR_ARG;
+    std::memcpy(dst, a->data(), n * sizeof(double));
+    return DRO_OK;
+}
+int dro_set_raw(dro_handle* H, int id, const double* src, size_t n) {
+    std::vector<double>* a = H ? raw_array(H, id) : nullptr;
+    if (!a || !src || n != a->size() || a->empty()) return DRO_ERR_ARG;
+    std::memcpy(a->data(), src, n * sizeof(double));
+    return DRO_OK;
+}
+
 const char* dro_last_error(dro_handle* H) { return H ? H->err.c_str() : "null handle"; }
 
 void dro_destroy(dro_handle* H) { delete H; }

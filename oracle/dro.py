@@ -55,6 +55,10 @@ def lib():
         L.dro_last_error.argtypes = [C.c_void_p]
         L.dro_last_error.restype = C.c_char_p
         L.dro_stop_reason.argtypes = [C.c_void_p]
+        L.dro_raw_size.argtypes = [C.c_void_p, C.c_int]
+        L.dro_raw_size.restype = C.c_size_t
+        L.dro_get_raw.argtypes = [C.c_void_p, C.c_int, dp, C.c_size_t]
+        L.dro_set_raw.argtypes = [C.c_void_p, C.c_int, dp, C.c_size_t]
         L.dro_destroy.argtypes = [C.c_void_p]
         L.dro_destroy.restype = None
         _lib = L
@@ -136,6 +140,22 @@ class Oracle:
         out = np.empty(self.field_shape(f))
         self._check(lib().dro_get_field(self._h, f, _dp(out), out.size))
         return out
+
+    RAW = ("vx", "vy", "vz", "p", "txx", "tyy", "tzz", "tyz", "txz", "txy")
+
+    def raw_shape(self, name):
+        return self.field_shape({"vx": 0, "vy": 1, "vz": 2, "p": 3, "txx": 3, "tyy": 3, "tzz": 3, "tyz": 6, "txz": 7, "txy": 8}[name])
+
+    def get_raw(self, name):
+        """the oracle's own state array (p and tau_aa separately, Eq. 10), for the z-slab halo test"""
+        out = np.empty(self.raw_shape(name))
+        self._check(lib().dro_get_raw(self._h, self.RAW.index(name), _dp(out), out.size))
+        return out
+
+    def set_raw(self, name, a):
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        assert a.shape == self.raw_shape(name)
+        self._check(lib().dro_set_raw(self._h, self.RAW.index(name), _dp(a), a.size))
 
     def solve_all(self, eps0=1e-4, tol=1e-8, maxiter=100000):
         """six load cases -> (C[6,6], [(status, iters, residual)]*6)"""

@@ -17,7 +17,7 @@ CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK, FORM, PALETTE, 
 STOP_NONE, STOP_RESIDUAL, STOP_STAGNATION, STOP_MAXITER = range(4)
 PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK, form=FORM, palette=PALETTE, stag_tol=STAG_TOL)
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
-EXPORTS = ("dr_workspace_bytes", "dr_create", "dr_set_param", "dr_solve", "dr_solve_six", "dr_effective_C_six", "dr_step", "dr_iterate",
+EXPORTS = ("dr_workspace_bytes", "dr_workspace_bytes_six", "dr_solve_all", "dr_info_lc", "dr_create", "dr_set_param", "dr_solve", "dr_solve_six", "dr_effective_C_six", "dr_step", "dr_iterate",
            "dr_effective_C", "dr_avg_stress", "dr_info", "dr_get_field", "dr_solve_image_host", "dr_contribution_tensor",
            "dr_uses_palette", "dr_active_kernel", "dr_stop_reason", "dr_launch_count", "dr_last_error", "dr_destroy")
 
@@ -35,6 +35,11 @@ def lib():
         dp, vp = C.POINTER(C.c_double), C.c_void_p
         L.dr_workspace_bytes.argtypes = [C.c_int] * 3
         L.dr_workspace_bytes.restype = C.c_size_t
+        if hasattr(L, "dr_workspace_bytes_six"):
+            L.dr_workspace_bytes_six.argtypes = [C.c_int] * 3
+            L.dr_workspace_bytes_six.restype = C.c_size_t
+            L.dr_solve_all.argtypes = [vp, C.c_double, C.c_double, C.c_int, C.POINTER(C.c_int)]
+            L.dr_info_lc.argtypes = [vp, C.c_int, C.POINTER(C.c_int), dp, C.POINTER(C.c_int)]
         L.dr_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, vp, vp, vp, C.c_size_t, vp, C.POINTER(vp)]
         L.dr_set_param.argtypes = [vp, C.c_int, C.c_double]
         L.dr_solve.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int]
@@ -73,8 +78,8 @@ class DrError(RuntimeError):
         self.status = status
 
 
-def workspace_bytes(nx, ny, nz):
-    return lib().dr_workspace_bytes(nx, ny, nz)
+def workspace_bytes(nx, ny, nz, six=False):
+    return lib().dr_workspace_bytes_six(nx, ny, nz) if six else lib().dr_workspace_bytes(nx, ny, nz)
 
 
 def field_shape(nx, ny, nz, f):
@@ -86,7 +91,7 @@ def field_shape(nx, ny, nz, f):
 class Solver:
     """dr_create .. dr_destroy.  K, G: torch.float64 CUDA tensors of shape (nz, ny, nx), x fastest."""
 
-    def __init__(self, K, G, h=1.0, stream=None, workspace=None, **params):
+    def __init__(self, K, G, h=1.0, stream=None, workspace=None, six=False, **params):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libdr needs a CUDA device (there is no CPU fallback)")
@@ -96,7 +101,7 @@ class Solver:
         self.nz, self.ny, self.nx = (int(s) for s in K.shape)
         self.device = K.device
         self._torch = torch
-        need = workspace_bytes(self.nx, self.ny, self.nz)
+        need = workspace_bytes(self.nx, self.ny, self.nz, six)
         if need == 0:
             raise DrError(ERR_ARG, "invalid grid size")
         if workspace is None:
@@ -171,6 +176,17 @@ class Solver:
     def launch_count(self):
         return lib().dr_launch_count(self._h)
 
+    def solve_all_batched(self, eps0=1e-4, tol=1e-8, maxiter=100000):
+        """dr_solve_all: six load cases per launch (Solver(..., six=True)).  Returns (C[6,6], [(status, iters, residual, stop)]*6)."""
+        stat = (C.c_int * 6)()
+        self._check(lib().dr_solve_all(self._h, eps0, tol, maxiter, stat), soft=(OK, MAXITER))
+        log = []
+        for lc in range(6):
+            it, r, sp = C.c_int(), C.c_double(), C.c_int()
+            lib().dr_info_lc(self._h, lc, C.byref(it), C.byref(r), C.byref(sp))
+            log.append((stat[lc], it.value, r.value, sp.value))
+        return self.effective_C(), log
+
     def solve_all(self, eps0=1e-4, tol=1e-8, maxiter=100000):
         log = []
         for lc in range(6):
@@ -230,7 +246,7 @@ def solve_six(K, G, h=1.0, eps0=1e-4, tol=1e-8, maxiter=100000, **params):
 
 
 def solve_image_host(K_host, G_host, h=1.0, eps0=1e-4, tol=1e-8, maxiter=100000, ncheck=0,
-                     stage=None, workspace=None, device="cuda:0"):
+                     stage=None, workspace=None, device="cuda:0", six=False):
     """End-to-end call with HOST arrays (numpy or CPU torch tensors, (nz,ny,nx) float64): host->device copies,
     six solves and the 6x6 result read back, all inside dr_solve_image_host.  Returns (C, iters, status)."""
     import numpy as np
@@ -243,7 +259,7 @@ def solve_image_host(K_host, G_host, h=1.0, eps0=1e-4, tol=1e-8, maxiter=100000,
     if stage is None:
         stage = torch.empty(2 * N, dtype=torch.float64, device=device)
     if workspace is None:
-        workspace = torch.empty(workspace_bytes(nx, ny, nz), dtype=torch.uint8, device=device)
+        workspace = torch.empty(workspace_bytes(nx, ny, nz, six), dtype=torch.uint8, device=device)
     Cout = np.zeros(36)
     iters = (C.c_int * 6)()
     with torch.cuda.device(stage.device):

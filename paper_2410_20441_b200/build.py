@@ -24,6 +24,19 @@ def _nvcc():
     return "nvcc"
 
 
+def source_hash():
+    """sha256 (first 16 hex digits) of the CUDA sources and the public header: identifies the kernels a profile under
+    profiles/ was taken with (bench.py emits roofline.traffic only for a matching hash)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(SOURCES + HEADERS):
+        with open(os.path.join(CSRC, f), "rb") as fh:
+            h.update(f.encode() + b"\0" + fh.read())
+    with open(os.path.join(HERE, "..", "include", "dr.h"), "rb") as fh:
+        h.update(b"dr.h\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
 def stale():
     if not os.path.exists(LIB):
         return True
@@ -49,4 +62,7 @@ def build(force=False, verbose=False):
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--hash" in sys.argv:
+        print(source_hash())
+    else:
+        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

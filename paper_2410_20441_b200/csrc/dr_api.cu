@@ -40,7 +40,7 @@ struct dr_handle {
     int use_pal;                // DR_PALETTE
     unsigned int* flags;
     // host
-    double* pinned;             // 16 doubles, page-locked: [0..5] averages, [8] residual, [9..14] averages at a check
+    double* pinned;             // 64 doubles, page-locked: [0..5] averages, [8] residual, [9..14] averages at a check; dr_solve_all: [16..21] residuals, [24..59] averages
     cudaEvent_t e0, e1;
     // parameters
     double cfl, st_factor, void_rel, stag_tol;
@@ -76,6 +76,14 @@ struct dr_handle {
     int tb2_lz;
     bool lz_user;               // DR_ZCHUNK set by the caller
     CUtensorMap tm2_state[2][F_COUNT];   // boxes TB2_TX x TB2_TY x 1
+    // six-load-case batch (dr_solve_all): state set q belongs to load case q; set 0 is the single-solve state above
+    int nsets;                  // 6 if the workspace holds six state sets (dr_workspace_bytes_six), else 1
+    double* xbuf[TB2_NLC][2][F_COUNT];
+    CUtensorMap xtm2[TB2_NLC][2][F_COUNT];
+    double* partial6;           // [6][DR_AVG_BLOCKS][6]
+    double* avg6_dev;           // [6][6]
+    int lc_iters[6], lc_stop[6];
+    double lc_res[6];
     std::string err;
 };
 
@@ -130,16 +138,24 @@ extern "C" size_t dr_workspace_bytes(int nx, int ny, int nz) {
     return (size_t)N_BIG * field_bytes(L) + ids_bytes(L) + SMALL_BYTES + codes_bytes(L) + CODE_SMALL_BYTES;
 }
 
+// five more state sets (2 x 9 fields each) and the reduction scratch of six simultaneous load cases
+static const size_t SIX_SMALL_BYTES = align_up((size_t)6 * DR_AVG_BLOCKS * 6 * sizeof(double), 256) + 512;
+extern "C" size_t dr_workspace_bytes_six(int nx, int ny, int nz) {
+    if (!sizes_ok(nx, ny, nz)) return 0;
+    DrLayout L = dr_make_layout(nx, ny, nz);
+    return dr_workspace_bytes(nx, ny, nz) + (size_t)5 * 2 * F_COUNT * field_bytes(L) + SIX_SMALL_BYTES;
+}
+
 // z-chunk length of the fused kernels: make the CTA count fill whole waves of 148 SMs while keeping the priming
 // overhead (one extra step per chunk) small.  Chunks are capped at DR_LZ_MAX layers (and may be as short as 1-3 layers on tiny grids, where filling the 148 SMs matters more than the priming step): measured on B200, CTAs of
 // neighbouring tiles drift apart on longer marches and the halo rows/columns they share stop hitting in L2
 // (479^3: 3.53 ms/iteration at 24-32 layers per chunk, 3.67 at 48, 4.37 at 64, 5.2 at 96).
 #define DR_LZ_MAX 36
 #define DR_LZ_FIXED 3      // per-CTA start-up (barrier init, first TMA round trip) in units of one z step
-static int choose_lz_for(int tiles, int layers, int priming) {
-    int best_lz = layers < DR_LZ_MAX ? layers : DR_LZ_MAX;
+static int choose_lz_for(int tiles, int layers, int priming, int lz_max) {
+    int best_lz = layers < lz_max ? layers : lz_max;
     double best = 1e300;
-    for (int lz = 1; lz <= DR_LZ_MAX && lz <= layers; ++lz) {
+    for (int lz = 1; lz <= lz_max && lz <= layers; ++lz) {
         const int chunks = (layers + lz - 1) / lz;
         const double waves = std::ceil((double)tiles * chunks / 148.0);
         const double cost = waves * (lz + priming + DR_LZ_FIXED);          // steps on the critical path of one SM
@@ -148,11 +164,13 @@ static int choose_lz_for(int tiles, int layers, int priming) {
     return best_lz;
 }
 static int choose_lz(const DrLayout& L) {
-    return choose_lz_for(tiles_x(L) * tiles_y(L), L.nz + 1, 1);
+    return choose_lz_for(tiles_x(L) * tiles_y(L), L.nz + 1, 1, DR_LZ_MAX);
 }
-// the two-iteration kernel runs lz + 4 steps per chunk (two priming steps per iteration)
+// the two-iteration kernel runs lz + 4 steps per chunk (two priming steps per iteration); it is not DRAM-bound, so longer
+// marches cost nothing in halo reuse (479^3: 2.57 ms per iteration at 32 layers, 2.52 at 60, flat beyond)
+#define DR_LZ_MAX_TB2 64
 static int choose_lz_tb2(const DrLayout& L) {
-    return choose_lz_for(tb2_tiles_x(L) * tb2_tiles_y(L), L.nz + 1, 4);
+    return choose_lz_for(tb2_tiles_x(L) * tb2_tiles_y(L), L.nz + 1, 4, DR_LZ_MAX_TB2);
 }
 
 // TMA descriptor of one padded field: 3-D fp64 tensor (PX,PY,PZ), box (FUSED_TX, FUSED_TY, 1), no swizzle,
@@ -184,6 +202,9 @@ static bool make_all_tmaps(dr_handle* H) {
     dr_encode_fn enc = (dr_encode_fn)fn;
     for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) if (!make_tmap(H, enc, &H->tm_state[b][f], H->buf[b][f])) return false;
     for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) if (!make_tmap(H, enc, &H->tm2_state[b][f], H->buf[b][f], TB2_TX, TB2_TY)) return false;
+    for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) H->xtm2[0][b][f] = H->tm2_state[b][f];
+    for (int q = 1; q < H->nsets; ++q) for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f)
+        if (!make_tmap(H, enc, &H->xtm2[q][b][f], H->xbuf[q][b][f], TB2_TX, TB2_TY)) return false;
     return make_tmap(H, enc, &H->tm_K, H->K) && make_tmap(H, enc, &H->tm_G, H->G);
 }
 
@@ -216,13 +237,23 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
     H->codes = (unsigned long long*)p; p += codes_bytes(H->L);
     H->ekeys = (unsigned long long*)p; p += 2048; H->rkeys = (unsigned long long*)p; p += 2048;
     H->tabs = (double*)p; p += TB2_TAB_N * sizeof(double);
+    for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) H->xbuf[0][b][f] = H->buf[b][f];
+    H->nsets = workspace_bytes >= dr_workspace_bytes_six(nx, ny, nz) ? 6 : 1;
+    H->partial6 = nullptr; H->avg6_dev = nullptr;
+    if (H->nsets == 6) {
+        p = (char*)align_up((size_t)p, 256);
+        for (int q = 1; q < 6; ++q) for (int b = 0; b < 2; ++b) for (int f = 0; f < F_COUNT; ++f) { H->xbuf[q][b][f] = (double*)p; p += fb; }
+        H->partial6 = (double*)p; p += align_up((size_t)6 * DR_AVG_BLOCKS * 6 * sizeof(double), 256);
+        H->avg6_dev = (double*)p; p += 512;
+    }
+    for (int q = 0; q < 6; ++q) { H->lc_iters[q] = 0; H->lc_stop[q] = DR_STOP_NONE; H->lc_res[q] = 0.0; }
     H->has_codes = false; H->codes_failed = false; H->code_gavg = -1; H->code_void = -1.0;
     H->tb2_lz = choose_lz_tb2(H->L); H->lz_user = false;
     H->has_pal = false; H->use_pal = 1;
     H->pinned = nullptr; H->e0 = H->e1 = nullptr;
     if (cudaGetDevice(&H->device) != cudaSuccess) { cudaGetLastError(); delete H; return DR_ERR_CUDA; }
     H->stag_tol = 1e-10; H->stop_reason = DR_STOP_NONE;
-    H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->kernel = 0; H->form = 0;
+    H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->kernel = 3; H->form = 0;
     H->void_applied = 0.0; H->hmax = 0.0;
     H->cur = 0; H->have_fields = false; H->cur_lc = -1; H->cur_eps0 = 0.0;
     for (int a = 0; a < 6; ++a) { H->have[a] = false; H->avg[a] = 0; for (int b = 0; b < 6; ++b) H->Ccol[a][b] = 0.0; }
@@ -231,10 +262,10 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
 
     dr_status st = DR_OK;
     do {
-        if (!cuda_ok(H, cudaMallocHost((void**)&H->pinned, 16 * sizeof(double)), "cudaMallocHost")) { st = DR_ERR_CUDA; break; }
+        if (!cuda_ok(H, cudaMallocHost((void**)&H->pinned, 64 * sizeof(double)), "cudaMallocHost")) { st = DR_ERR_CUDA; break; }
         if (!cuda_ok(H, cudaEventCreate(&H->e0), "cudaEventCreate") || !cuda_ok(H, cudaEventCreate(&H->e1), "cudaEventCreate")) { st = DR_ERR_CUDA; break; }
         // state fields and moduli boxes start as zeros (halo nodes are never written afterwards)
-        if (!cuda_ok(H, cudaMemsetAsync(workspace, 0, dr_workspace_bytes(nx, ny, nz), H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }
+        if (!cuda_ok(H, cudaMemsetAsync(workspace, 0, H->nsets == 6 ? dr_workspace_bytes_six(nx, ny, nz) : dr_workspace_bytes(nx, ny, nz), H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }
         if (!cuda_ok(H, cudaMemsetAsync(H->palK, 0xff, 4096, H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }     // palK and palG := EMPTY
         dim3 blk(64, 4, 1), grd((nx + 2 + 63) / 64, (ny + 2 + 3) / 4, nz + 2);
         k_pad_moduli<<<grd, blk, 0, H->st>>>(H->L, K, G, H->K0, H->G0, H->flags, H->hmax_bits);
@@ -386,7 +417,8 @@ static dr_status ensure_codes(dr_handle* H) {
     return DR_OK;
 }
 
-static dr_status prepare(dr_handle* H, int lc, double eps0) {
+// moduli-side preparation of a solve: the void clamp and, for the coded kernels, the stencil codes
+static dr_status prepare_moduli(dr_handle* H) {
     const DrLayout& L = H->L;
     if (H->void_applied != H->void_rel) {
         k_void_clamp<<<(unsigned)((L.count + 255) / 256), 256, 0, H->st>>>(H->L, H->K0, H->G0, H->K, H->G, H->void_rel * H->hmax);
@@ -394,11 +426,16 @@ static dr_status prepare(dr_handle* H, int lc, double eps0) {
         if (H->has_pal) { k_pal_values<<<1, 256, 0, H->st>>>(H->palK, H->palG, H->pal, H->void_rel * H->hmax); CKL("k_pal_values"); }
         H->void_applied = H->void_rel;
     }
-    if (H->kernel >= 3) {
-        if (H->form == 1) return fail(H, DR_ERR_ARG, "DR_FORM = 1 is implemented by DR_KERNEL 0 and 1 only");
+    if (H->kernel >= 3 && H->form == 0) {          // the displacement form runs the one-sweep TMA kernel
         dr_status cs = ensure_codes(H);
         if (cs != DR_OK) return cs;
     }
+    return DR_OK;
+}
+
+static dr_status prepare(dr_handle* H, int lc, double eps0) {
+    const DrLayout& L = H->L;
+    { dr_status ms = prepare_moduli(H); if (ms != DR_OK) return ms; }
     DrPT P = make_pt(H, lc, eps0);
     dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
     if (H->form == 1 && H->kernel == 2) return fail(H, DR_ERR_ARG, "DR_FORM = 1 is implemented by DR_KERNEL 0 and 1 only");
@@ -412,24 +449,39 @@ static dr_status prepare(dr_handle* H, int lc, double eps0) {
 // the coded kernels (DR_KERNEL 3, 4) need the stencil codes; without them the one-sweep TMA kernel runs
 static bool coded(const dr_handle* H) { return H->kernel >= 3 && H->has_codes && H->form == 0; }
 
-// nit PT iterations in one sweep of the coded kernel (dr_kernels_tb2.cuh); with_res: residual of the LAST of them
-static dr_status iteration_coded(dr_handle* H, const DrPT& P, bool with_res, int nit) {
+// slot `slot` of a batch launch <- state set `set` (old state in its buffer `cur`, new state into the other one)
+static void fill_slot(dr_handle* H, DrTb2Batch& TB, int slot, int set, int cur, const DrPT& P) {
+    static const int order[9] = {F_VX, F_VY, F_VZ, F_SXX, F_SYY, F_SZZ, F_TXY, F_TXZ, F_TYZ};
+    for (int f = 0; f < 9; ++f) TB.m[slot][f] = H->xtm2[set][cur][order[f]];
+    TB.out[slot] = H->xbuf[set][cur ^ 1][0];
+    TB.res[slot] = H->res_bits + set;
+    TB.P[slot] = P;
+}
+
+// launch the coded kernel on the first nslots slots of TB: nit PT iterations per sweep; with_res: residual of the last
+static dr_status launch_coded(dr_handle* H, DrTb2Batch& TB, int nslots, bool with_res, int nit) {
     const DrLayout& L = H->L;
     const int lz = H->tb2_lz;
-    dim3 blk(TB2_TX, TB2_TY, 1), grd(tb2_tiles_x(L), tb2_tiles_y(L), (L.nz + 1 + lz - 1) / lz);
-    DrTb2Maps T;
-    const int c = H->cur;
-    static const int order[9] = {F_VX, F_VY, F_VZ, F_SXX, F_SYY, F_SZZ, F_TXY, F_TXZ, F_TYZ};
-    for (int f = 0; f < 9; ++f) T.m[f] = H->tm2_state[c][order[f]];
-    T.codes = H->codes; T.tabs = H->tabs; T.gx = (int)grd.x; T.gy = (int)grd.y;
-    T.l2_hint = 0x1000000000000000ull;
+    const int nchunks = (L.nz + 1 + lz - 1) / lz;
+    dim3 blk(TB2_TX, TB2_TY, 1), grd(tb2_tiles_x(L), tb2_tiles_y(L), nchunks * nslots);
+    TB.fs = H->buf[0][1] - H->buf[0][0];
+    TB.codes = H->codes; TB.tabs = H->tabs; TB.gx = (int)grd.x; TB.gy = (int)grd.y; TB.nchunks = nchunks;
+    TB.l2_hint = 0x1000000000000000ull;
     const size_t smem = DrTb2Cfg<TB2_TX, TB2_TY>::SMEM;
-    DrFields Bo = fields_of(H, c ^ 1);
-    if (nit == 2) { if (with_res) k_pt_tb2<1, 2, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(T, H->L, P, Bo, lz, H->res_bits);
-                    else          k_pt_tb2<0, 2, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); }
-    else          { if (with_res) k_pt_tb2<1, 1, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(T, H->L, P, Bo, lz, H->res_bits);
-                    else          k_pt_tb2<0, 1, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(T, H->L, P, Bo, lz, H->res_bits); }
+    if (nit == 2) { if (with_res) k_pt_tb2<1, 2, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(TB, H->L, lz);
+                    else          k_pt_tb2<0, 2, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(TB, H->L, lz); }
+    else          { if (with_res) k_pt_tb2<1, 1, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(TB, H->L, lz);
+                    else          k_pt_tb2<0, 1, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(TB, H->L, lz); }
     CKL("k_pt_tb2");
+    return DR_OK;
+}
+
+// nit PT iterations in one sweep of the coded kernel (dr_kernels_tb2.cuh); with_res: residual of the LAST of them
+static dr_status iteration_coded(dr_handle* H, const DrPT& P, bool with_res, int nit) {
+    static thread_local DrTb2Batch TB;
+    fill_slot(H, TB, 0, 0, H->cur, P);
+    dr_status s = launch_coded(H, TB, 1, with_res, nit);
+    if (s != DR_OK) return s;
     H->cur ^= 1;
     return DR_OK;
 }
@@ -437,8 +489,8 @@ static dr_status iteration_coded(dr_handle* H, const DrPT& P, bool with_res, int
 // one PT iteration; with_res: also accumulate the residual max-norm into res_bits (caller zeroes it)
 static dr_status iteration(dr_handle* H, const DrPT& P, bool with_res) {
     const DrLayout& L = H->L;
-    if (H->kernel == 4 && coded(H)) return iteration_coded(H, P, with_res, 1);
-    const int kernel = H->kernel >= 3 ? 0 : H->kernel;      // DR_KERNEL 3 single sweeps, and uncoded images: the TMA kernel
+    if (coded(H)) return iteration_coded(H, P, with_res, 1);  // DR_KERNEL 4, and the odd single sweeps of DR_KERNEL 3
+    const int kernel = H->kernel >= 3 ? 0 : H->kernel;      // uncoded images and the displacement form: the TMA kernel
     if (kernel == 1) {
         dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
         // FORM 0: in place in buffer cur.  FORM 1: u, w in buffer cur, stresses of this iteration in buffer cur^1.
@@ -708,6 +760,125 @@ extern "C" dr_status dr_effective_C_six(dr_handle* const h[6], double out[36]) {
     return DR_OK;
 }
 
+// the six load cases of one image advanced TOGETHER -- every launch of the two-iteration kernel
+// carries all unfinished load cases (they share the stencil codes; one direct test per stiffness column).
+// Same iterates, residual checks, stagnation rule and C as six dr_solve calls.
+extern "C" dr_status dr_solve_all(dr_handle* H, double eps0, double tol, int maxiter, int status_out[6]) {
+    if (!H) return DR_ERR_ARG;
+    DrDeviceGuard dg(H->device);
+    if (bad_lc(H, 0, eps0)) return DR_ERR_ARG;
+    if (!(tol > 0.0) || maxiter < 1) return fail(H, DR_ERR_ARG, "bad tol or maxiter");
+    if (H->nsets != 6) return fail(H, DR_ERR_WORKSPACE, "dr_solve_all needs a workspace of dr_workspace_bytes_six() bytes at dr_create");
+    CK(cudaEventRecord(H->e0, H->st));
+    { dr_status ms = prepare_moduli(H); if (ms != DR_OK) return ms; }
+    dr_status worst = DR_OK;
+    if (!(H->kernel == 3 && coded(H))) {
+        // not a stencil-coded image (or another kernel / form chosen): the six solves one after the other on state set 0
+        cudaEvent_t keep = H->e0;
+        for (int lc = 0; lc < 6; ++lc) {
+            dr_status s = dr_solve(H, lc, eps0, tol, maxiter);
+            H->lc_iters[lc] = H->iters; H->lc_res[lc] = H->residual; H->lc_stop[lc] = H->stop_reason;
+            if (status_out) status_out[lc] = (int)s;
+            if (s != DR_OK && s != DR_MAXITER) return s;
+            if (s == DR_MAXITER) worst = DR_MAXITER;
+        }
+        (void)keep;
+        return worst;
+    }
+    const DrLayout& L = H->L;
+    DrPT P[6];
+    int cur[6];
+    bool active[6];
+    dr_status st[6];
+    DrStag stag[6];
+    for (int lc = 0; lc < 6; ++lc) {
+        P[lc] = make_pt(H, lc, eps0);
+        DrFields F; for (int f = 0; f < F_COUNT; ++f) F.f[f] = H->xbuf[lc][0][f];
+        dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
+        if (H->gavg) k_bc_init<1><<<grd, blk, 0, H->st>>>(H->L, P[lc], F, F, 0, H->K, H->G);
+        else         k_bc_init<0><<<grd, blk, 0, H->st>>>(H->L, P[lc], F, F, 0, H->K, H->G);
+        CKL("k_bc_init");
+        cur[lc] = 0; active[lc] = true; st[lc] = DR_MAXITER;
+        H->lc_iters[lc] = 0; H->lc_res[lc] = INFINITY; H->lc_stop[lc] = DR_STOP_MAXITER; H->have[lc] = false;
+    }
+    H->have_fields = false;                          // set 0 now holds load case 0 of the batch, not a dr_step state
+    static thread_local DrTb2Batch TB;
+    const bool use_stag = H->stag_tol > 0.0;
+    const double invN = 1.0 / ((double)L.nx * L.ny * L.nz);
+    int it = 0, nact = 6;
+    while (nact > 0 && it < maxiter) {
+        const int n = (it + 2 <= maxiter && (it + 1) % H->ncheck != 0) ? 2 : 1;
+        it += n;
+        const bool chk = (it % H->ncheck == 0);
+        int slots[6], ns = 0;
+        for (int lc = 0; lc < 6; ++lc) if (active[lc]) { fill_slot(H, TB, ns, lc, cur[lc], P[lc]); slots[ns++] = lc; }
+        if (chk) CK(cudaMemsetAsync(H->res_bits, 0, 6 * 8, H->st));
+        { dr_status s = launch_coded(H, TB, ns, chk, n); if (s != DR_OK) return s; }
+        for (int a = 0; a < ns; ++a) cur[slots[a]] ^= 1;
+        if (!chk) continue;
+        if (use_stag) {
+            DrAvgSix A;
+            for (int a = 0; a < ns; ++a) for (int f = 0; f < F_COUNT; ++f) A.F[a].f[f] = H->xbuf[slots[a]][cur[slots[a]]][f];
+            k_avg_partial6<<<dim3(DR_AVG_BLOCKS, ns), DR_AVG_THREADS, 0, H->st>>>(H->L, A, H->partial6);
+            CKL("k_avg_partial6");
+            k_avg_final6<<<ns, 256, 0, H->st>>>(H->partial6, DR_AVG_BLOCKS, invN, H->avg6_dev);
+            CKL("k_avg_final6");
+            CK(cudaMemcpyAsync(H->pinned + 24, H->avg6_dev, (size_t)ns * 6 * sizeof(double), cudaMemcpyDeviceToHost, H->st));
+        }
+        CK(cudaMemcpyAsync(H->pinned + 16, H->res_bits, 6 * 8, cudaMemcpyDeviceToHost, H->st));
+        CK(cudaStreamSynchronize(H->st));
+        for (int a = 0; a < ns; ++a) {
+            const int lc = slots[a];
+            double r;
+            std::memcpy(&r, H->pinned + 16 + lc, 8);
+            H->lc_res[lc] = r;
+            bool done = false;
+            if (!std::isfinite(r)) { st[lc] = DR_ERR_DIVERGED; H->lc_stop[lc] = DR_STOP_NONE; done = true; }
+            else if (r <= tol) { st[lc] = DR_OK; H->lc_stop[lc] = DR_STOP_RESIDUAL; done = true; }
+            else if (use_stag && stag[lc].update(H->pinned + 24 + 6 * a, H->stag_tol)) { st[lc] = DR_OK; H->lc_stop[lc] = DR_STOP_STAGNATION; done = true; }
+            if (done) { active[lc] = false; H->lc_iters[lc] = it; --nact; }
+        }
+    }
+    for (int lc = 0; lc < 6; ++lc) if (active[lc]) H->lc_iters[lc] = it;
+    // volume averages of all six final states (Eq. 7) -> the six columns (Eq. 9, 22)
+    {
+        DrAvgSix A;
+        for (int lc = 0; lc < 6; ++lc) for (int f = 0; f < F_COUNT; ++f) A.F[lc].f[f] = H->xbuf[lc][cur[lc]][f];
+        k_avg_partial6<<<dim3(DR_AVG_BLOCKS, 6), DR_AVG_THREADS, 0, H->st>>>(H->L, A, H->partial6);
+        CKL("k_avg_partial6");
+        k_avg_final6<<<6, 256, 0, H->st>>>(H->partial6, DR_AVG_BLOCKS, invN, H->avg6_dev);
+        CKL("k_avg_final6");
+        CK(cudaMemcpyAsync(H->pinned + 24, H->avg6_dev, 36 * sizeof(double), cudaMemcpyDeviceToHost, H->st));
+        CK(cudaEventRecord(H->e1, H->st));
+        CK(cudaStreamSynchronize(H->st));
+    }
+    for (int lc = 0; lc < 6; ++lc) {
+        if (status_out) status_out[lc] = (int)st[lc];
+        if (st[lc] == DR_ERR_DIVERGED) { worst = DR_ERR_DIVERGED; continue; }
+        for (int m = 0; m < 6; ++m) H->Ccol[lc][m] = H->pinned[24 + 6 * lc + m] / eps0;
+        H->have[lc] = true;
+        if (st[lc] == DR_MAXITER && worst == DR_OK) worst = DR_MAXITER;
+    }
+    for (int m = 0; m < 6; ++m) H->avg[m] = H->pinned[24 + 30 + m];
+    H->have_avg = true;
+    H->iters = H->lc_iters[5]; H->residual = H->lc_res[5]; H->stop_reason = H->lc_stop[5];
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, H->e0, H->e1));
+    H->ms = ms;
+    if (worst == DR_MAXITER) H->err = "maxiter reached";
+    if (worst == DR_ERR_DIVERGED) H->err = "residual is not finite";
+    return worst;
+}
+
+// iterations, last residual and dr_stop of load case lc in the last dr_solve_all
+extern "C" dr_status dr_info_lc(dr_handle* H, int lc, int* iters, double* residual, int* stop) {
+    if (!H || lc < 0 || lc > 5) return DR_ERR_ARG;
+    if (iters) *iters = H->lc_iters[lc];
+    if (residual) *residual = H->lc_res[lc];
+    if (stop) *stop = H->lc_stop[lc];
+    return DR_OK;
+}
+
 extern "C" dr_status dr_step(dr_handle* H, int lc, double eps0, int niter) {
     if (!H) return DR_ERR_ARG;
     DrDeviceGuard dg(H->device);
@@ -805,6 +976,12 @@ extern "C" dr_status dr_solve_image_host(int nx, int ny, int nz, double h, const
     if (s != DR_OK) return s;
     dr_status worst = DR_OK;
     if (ncheck > 0) dr_set_param(H, DR_NCHECK, ncheck);
+    if (H->nsets == 6) {                             // workspace of dr_workspace_bytes_six: all six load cases per launch
+        s = dr_solve_all(H, eps0, tol, maxiter, nullptr);
+        if (iters_out) for (int lc = 0; lc < 6; ++lc) iters_out[lc] = H->lc_iters[lc];
+        if (s != DR_OK && s != DR_MAXITER) { dr_destroy(H); return s; }
+        worst = s;
+    } else
     for (int lc = 0; lc < 6; ++lc) {
         s = dr_solve(H, lc, eps0, tol, maxiter);
         if (iters_out) iters_out[lc] = H->iters;

@@ -178,6 +178,45 @@ k_avg_partial(DrLayout L, DrConstFields F, double* __restrict__ partial) {
     }
 }
 
+// the same two passes for up to six state sets at once (dr_solve_all): blockIdx.y = slot
+struct DrAvgSix { DrConstFields F[6]; };
+
+__global__ void __launch_bounds__(DR_AVG_THREADS)
+k_avg_partial6(DrLayout L, DrAvgSix A, double* __restrict__ partial6) {
+    const DrConstFields& F = A.F[blockIdx.y];
+    double* partial = partial6 + (size_t)blockIdx.y * DR_AVG_BLOCKS * 6;
+    const int nx = L.nx, ny = L.ny, nz = L.nz;
+    const long long rows = (long long)(ny + 1) * (nz + 1);
+    double s[6] = {0, 0, 0, 0, 0, 0};
+    for (long long r = blockIdx.x; r < rows; r += gridDim.x) {
+        int j = (int)(r % (ny + 1)), k = (int)(r / (ny + 1));
+        const bool cj = j < ny, ck = k < nz;
+        const double wj = (j == 0 || j == ny) ? 0.5 : 1.0, wk = (k == 0 || k == nz) ? 0.5 : 1.0;
+        long long q0 = L.origin + L.sy * j + L.sz * k;
+        for (int i = threadIdx.x; i <= nx; i += blockDim.x) {
+            long long q = q0 + i;
+            const bool ci = i < nx;
+            const double wi = (i == 0 || i == nx) ? 0.5 : 1.0;
+            if (ci && cj && ck) { s[0] += F.f[F_SXX][q]; s[1] += F.f[F_SYY][q]; s[2] += F.f[F_SZZ][q]; }
+            if (ci) s[3] += wj * wk * F.f[F_TYZ][q];
+            if (cj) s[4] += wi * wk * F.f[F_TXZ][q];
+            if (ck) s[5] += wi * wj * F.f[F_TXY][q];
+        }
+    }
+    __shared__ double sm[6][DR_AVG_THREADS / 32];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+        double v = dr_warp_sum(s[m]);
+        if ((threadIdx.x & 31) == 0) sm[m][threadIdx.x >> 5] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        double v = 0;
+        for (int w = 0; w < DR_AVG_THREADS / 32; ++w) v += sm[threadIdx.x][w];
+        partial[(size_t)blockIdx.x * 6 + threadIdx.x] = v;
+    }
+}
+
 __global__ void __launch_bounds__(256) k_avg_final(const double* __restrict__ partial, int nblocks, double invN, double* out6) {
     __shared__ double sm[6][256];
     double s[6] = {0, 0, 0, 0, 0, 0};
@@ -280,4 +319,20 @@ __global__ void k_pal_values(const unsigned long long* __restrict__ kK, const un
         if (thr > 0.0 && Kv + 4.0 * Gv / 3.0 <= thr) { Kv = 0.0; Gv = 0.0; }
     }
     pal[e] = Kv; pal[256 + e] = Gv;
+}
+
+// second pass for six sets: block b reduces the partials of slot b into out36[6 * b .. 6 * b + 5] (same order as k_avg_final)
+__global__ void __launch_bounds__(256) k_avg_final6(const double* __restrict__ partial6, int nblocks, double invN, double* out36) {
+    const double* partial = partial6 + (size_t)blockIdx.x * nblocks * 6;
+    __shared__ double sm[6][256];
+    double s[6] = {0, 0, 0, 0, 0, 0};
+    for (int b = threadIdx.x; b < nblocks; b += 256)
+        for (int m = 0; m < 6; ++m) s[m] += partial[(size_t)b * 6 + m];
+    for (int m = 0; m < 6; ++m) sm[m][threadIdx.x] = s[m];
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) for (int m = 0; m < 6; ++m) sm[m][threadIdx.x] += sm[m][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x < 6) out36[6 * blockIdx.x + threadIdx.x] = sm[threadIdx.x][0] * invN;
 }

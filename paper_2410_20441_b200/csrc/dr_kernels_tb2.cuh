@@ -36,23 +36,49 @@
 #define TB2_TX 32
 #endif
 #ifndef TB2_TY
-#define TB2_TY 14
+#define TB2_TY 16
+#endif
+#ifndef TB2_UNROLL4
+#define TB2_UNROLL4 0      // 1: march unrolled by 4 (every ring slot a compile-time constant); 0: by 2 (ring-A slot at run time)
+#endif
+#ifndef TB2_REREAD
+#define TB2_REREAD 0       // 1: B2 reads its own second-iteration stresses back from the exchange planes; 0: keeps them in registers
 #endif
 #define TB2_KLO 2          // coded layers below layer 0 (layers -2, -1) ...
 #define TB2_KHI 3          // ... and above layer nz-1 (layers nz, nz+1, nz+2)
 
-// tables of one coded image: K[256] G[256] (cell palette, after the void clamp), E[256] edge moduli, R[256] 1/H_node
+// tables of one coded image (global memory): K[256] G[256] (cell palette, after the void clamp), E[256] edge moduli,
+// R[256] 1/H_node
 #define TB2_TAB_K 0
 #define TB2_TAB_G 256
 #define TB2_TAB_E 512
 #define TB2_TAB_R 768
 #define TB2_TAB_N 1024
+// what a CTA derives from them once, in shared memory: the products that are the same in every iteration
+//   LAM = K - 2G/3,  G2 = 2G,  ES = (theta/h) E,  CV = (C~^2 h^2 / (theta h)) R,  RH = R (residual launches only)
+#define TB2_S_LAM 0
+#define TB2_S_G2 256
+#define TB2_S_ES 512
+#define TB2_S_CV 768
+#define TB2_S_RH 1024
 
-struct DrTb2Maps {
-    CUtensorMap m[9];                     // vx vy vz | sxx syy szz txy | txz tyz   (old state, boxes TX x TY x 1)
+// One launch advances up to six load cases of the same image ("slots"; they share the stencil codes and tables, P:142-149:
+// one direct test per stiffness column): blockIdx.z = slot * nchunks + z chunk.  A single solve is a batch of one.
+#define TB2_NLC 6
+struct DrTb2Batch {
+    CUtensorMap m[TB2_NLC][9];            // per slot: vx vy vz | sxx syy szz txy | txz tyz of the OLD state (boxes TX x TY x 1)
+    double* out[TB2_NLC];                 // per slot: field 0 (vx) of the NEW state; the other fields follow at stride fs
+    unsigned long long* res[TB2_NLC];     // per slot: residual max-norm (bit pattern, atomicMax)
+    DrPT P[TB2_NLC];                      // per slot: constants of its load case
+    long long fs;                         // doubles between consecutive fields of a state buffer
     const unsigned long long* codes;      // [nz + KLO + KHI][gy][gx][TY][TX] stencil codes, layer -KLO first
     const double* tabs;                   // TB2_TAB_N doubles
-    int gx, gy;
+    int gx, gy, nchunks;
+    unsigned long long l2_hint;
+};
+// what the march needs of one slot
+struct DrTb2Maps {
+    const CUtensorMap* m;
     unsigned long long l2_hint;
 };
 
@@ -68,8 +94,8 @@ struct DrTb2Cfg {
     static constexpr int NB = 6;                             // ring B slot: sxx syy szz txy (layer m-1), txz tyz (face m)
     static constexpr int FRONT = 128;
     static constexpr int RING_A = FRONT;                     // [4][NA][PL]
-    static constexpr int RING_B = RING_A + 4 * NA * PL;      // [3][NB][PL]
-    static constexpr int X1 = RING_B + 3 * NB * PL;          // [2][Y_COUNT][PL]
+    static constexpr int RING_B = RING_A + 4 * NA * PL;      // [2][NB][PL]
+    static constexpr int X1 = RING_B + 2 * NB * PL;          // [2][Y_COUNT][PL]
     static constexpr int V1 = X1 + 2 * Y_COUNT * PL;         // [2][3][PL]
     static constexpr int X2 = V1 + 2 * 3 * PL;               // [Z_COUNT][PL]
     static constexpr int END = X2 + Z_COUNT * PL;
@@ -83,25 +109,25 @@ struct DrFace5 { double txz, tyz, szz, txz_r, tyz_u; };        // face values ca
 
 // Stage A of one PT iteration at node column (i,j), layer k (Eq. 12-13, relaxation term implicit): new normal
 // stresses and tau_xy of layer k, tau_xz / tau_yz of face k+1, from the velocities of layers k ("c") and k+1 ("n").
-// Same expressions, in the same order, as stage A of dr_tma_step (FORM 0).
+// Same expressions as stage A of dr_tma_step (FORM 0), except that the 1/h of the strain rates is folded into the
+// constants (thh = theta/h, es = theta/h x edge modulus): identical bits for h = 1, last-bit differences otherwise.
 template <bool BND>
 __device__ __forceinline__ DrStress6 dr_tb2_stress(const DrPT& P, const int nx, const int ny, const int nz,
                                                    const int i, const int j, const int k,
-                                                   const double Kc, const double Gc, const double gxy, const double gxz, const double gyz,
+                                                   const double lam, const double g2, const double esxy, const double esxz, const double esyz,
                                                    const double vxc, const double vyc, const double vzc,
                                                    const double vx_r, const double vy_u, const double vx_d, const double vy_l,
                                                    const double vxn, const double vyn, const double vzn,
                                                    const double vzn_l, const double vzn_d, const DrStress6& o) {
-    const double h = P.h, ih = P.inv_h, th = P.theta, ri = P.rinv;
+    const double h = P.h, ri = P.rinv, thh = P.theta * P.inv_h;
     DrStress6 n;
-    const double dxx = (vx_r - vxc) * ih;
-    const double dyy = (vy_u - vyc) * ih;
-    const double dzz = (vzn - vzc) * ih;
-    const double lam_div = fma(-(2.0 / 3.0), Gc, Kc) * (dxx + dyy + dzz);
-    const double g2 = 2.0 * Gc;
-    n.sxx = (o.sxx + th * fma(g2, dxx, lam_div)) * ri;
-    n.syy = (o.syy + th * fma(g2, dyy, lam_div)) * ri;
-    n.szz = (o.szz + th * fma(g2, dzz, lam_div)) * ri;
+    const double dxx = vx_r - vxc;
+    const double dyy = vy_u - vyc;
+    const double dzz = vzn - vzc;
+    const double lam_div = lam * (dxx + dyy + dzz);
+    n.sxx = (o.sxx + thh * fma(g2, dxx, lam_div)) * ri;
+    n.syy = (o.syy + thh * fma(g2, dyy, lam_div)) * ri;
+    n.szz = (o.szz + thh * fma(g2, dzz, lam_div)) * ri;
     double exy = (vxc - vx_d) + (vyc - vy_l);
     double exz = (vxn - vxc) + (vzn - vzn_l);
     double eyz = (vyn - vyc) + (vzn - vzn_d);
@@ -130,47 +156,69 @@ __device__ __forceinline__ DrStress6 dr_tb2_stress(const DrPT& P, const int nx, 
             + dr_dshear(vzn, vzn_d, j, ny, dr_u0(P, 2, x, j == 0 ? 0.0 : P.Ly, (k + 1) * h));
         zyz = false;
     }
-    n.txy = zxy ? 0.0 : (o.txy + th * gxy * (exy * ih)) * ri;
-    n.txz = zxz ? 0.0 : (o.txz + th * gxz * (exz * ih)) * ri;
-    n.tyz = zyz ? 0.0 : (o.tyz + th * gyz * (eyz * ih)) * ri;
+    n.txy = zxy ? 0.0 : fma(esxy, exy, o.txy) * ri;
+    n.txz = zxz ? 0.0 : fma(esxz, exz, o.txz) * ri;
+    n.tyz = zyz ? 0.0 : fma(esyz, eyz, o.tyz) * ri;
     return n;
 }
 
-// velocity update of one node (Eq. 11): v += C~^2 h^2 / (theta H_node) F; rH = 1/H_node from the table, 0 for wall,
-// dead and out-of-domain nodes (never updated, not part of the residual)
+// velocity update of one node (Eq. 11): v += C~^2 h^2 / (theta H_node) F, with F = Fh / h the stress divergence;
+// cv = C~^2 h^2 / (theta h H_node) and rH = 1/H_node from the tables, both 0 for wall, dead and out-of-domain nodes
+// (never updated, not part of the residual).  rmax collects |Fh| / H_node (scaled by 1/h and h/|eps0| at the end).
 template <int RES>
-__device__ __forceinline__ double dr_tb2_vel(const double v, const double F, const double rH, const double c2t, double& rmax, bool& rnan) {
-    if (rH != 0.0) {
-        if (RES) { const double r = fabs(F) * rH; rnan |= !(r == r); rmax = dr_max(rmax, r); }
-        return fma(c2t * rH, F, v);
+__device__ __forceinline__ double dr_tb2_vel(const double v, const double Fh, const double* tab, const unsigned idx8, double& rmax, bool& rnan) {
+    const double cv = *reinterpret_cast<const double*>(reinterpret_cast<const char*>(tab + TB2_S_CV) + idx8);
+    if (RES) {
+        const double r = fabs(Fh) * *reinterpret_cast<const double*>(reinterpret_cast<const char*>(tab + TB2_S_RH) + idx8);
+        if (cv != 0.0) { rnan |= !(r == r); rmax = dr_max(rmax, r); }
     }
-    return v;
+    return cv != 0.0 ? fma(cv, Fh, v) : v;
 }
 
-// one batch: ring-A planes of layer m (velocities + codes) and, if with_b, the ring-B set m (stresses of layer m-1, face m)
+// byte b of a stencil code as a byte offset into a table of doubles
+__device__ __forceinline__ unsigned dr_code_off(const unsigned long long c, const int b) {
+    return b == 0 ? ((unsigned)c << 3) & 0x7f8u : (unsigned)(c >> (8 * b - 3)) & 0x7f8u;
+}
+__device__ __forceinline__ double dr_tab_at(const double* tab, const unsigned off8) {
+    return *reinterpret_cast<const double*>(reinterpret_cast<const char*>(tab) + off8);
+}
+
+// TMA group u (u >= 0): what step u needs and no earlier step has brought: ring-A planes of layer m = k_u + 1 (velocities +
+// codes; slot (u+1) & 3) and the old stresses of step u (sxx syy szz txy of layer m-1, txz tyz of face m; ring-B slot u & 1).
+// Group -1 is ring-A layer kb-2 alone.  Completion: mbarrier (u+1) & 3, phase ((u+1) >> 2) & 1.
 template <int TX, int TY>
-__device__ __forceinline__ void dr_tb2_issue_batch(const DrTb2Maps& T, unsigned long long* bar, double* da, double* db,
+__device__ __forceinline__ void dr_tb2_issue_group(const DrTb2Maps& T, unsigned long long* bars, double* sm,
                                                    const unsigned long long* codesrc, long long codestride,
-                                                   int x0, int y0, int m, bool with_b) {
+                                                   int x0, int y0, int u, int m) {
     using Cfg = DrTb2Cfg<TX, TY>;
     constexpr int PL = Cfg::PL;
+    const bool with_b = u >= 0;
+    unsigned long long* bar = bars + ((u + 1) & 3);
+    double* da = sm + Cfg::RING_A + ((u + 1) & 3) * (Cfg::NA * PL);
+    double* db = sm + Cfg::RING_B + (u & 1) * (Cfg::NB * PL);
     dr_mbar_expect_tx(bar, with_b ? Cfg::BYTES_A + Cfg::BYTES_B : Cfg::BYTES_A);
 #pragma unroll
-    for (int f = 0; f < 3; ++f) dr_tma_load_3d(da + f * PL, &T.m[f], bar, x0, y0, m + 1, T.l2_hint);
+    for (int f = 0; f < 3; ++f) dr_tma_load_3d(da + f * PL, T.m + f, bar, x0, y0, m + 1, T.l2_hint);
     dr_bulk_load_1d(da + 3 * PL, codesrc + codestride * (m + TB2_KLO), PL * sizeof(double), bar);
     if (with_b) {
 #pragma unroll
-        for (int f = 0; f < 4; ++f) dr_tma_load_3d(db + f * PL, &T.m[3 + f], bar, x0, y0, m, T.l2_hint);
-        dr_tma_load_3d(db + 4 * PL, &T.m[7], bar, x0, y0, m + 1, T.l2_hint);
-        dr_tma_load_3d(db + 5 * PL, &T.m[8], bar, x0, y0, m + 1, T.l2_hint);
+        for (int f = 0; f < 4; ++f) dr_tma_load_3d(db + f * PL, T.m + 3 + f, bar, x0, y0, m, T.l2_hint);
+        dr_tma_load_3d(db + 4 * PL, T.m + 7, bar, x0, y0, m + 1, T.l2_hint);
+        dr_tma_load_3d(db + 5 * PL, T.m + 8, bar, x0, y0, m + 1, T.l2_hint);
     }
 }
 
-// step t of the march: first-iteration layer k = kb - 2 + t, second-iteration layer k2 = k - 2.  PAR = t & 1.
+// output: the 9 fields of the new state sit at a constant stride (fs doubles) in the workspace, in the order of dr_layout.cuh
+// (vx vy vz sxx syy szz tyz txz txy); col = this thread's node column in field 0.  One pointer instead of nine.
+struct DrTb2Out { double* col; long long fs; };
+
+// step t of the march: first-iteration layer k = kb - 2 + t, second-iteration layer k2 = k - 2.  Q = t & 3 is a template
+// parameter so that every shared-memory offset (ring slots, parity buffers) is a compile-time constant relative to the
+// thread's own address: the compiler can then interleave the four stages freely.
 // code2: in = stencil code of layer k-2 (stored by step t-2, same parity), out = that of layer k.
-template <int RES, int NIT, int TX, int TY, bool BND, int PAR>
-__device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, const DrTb2Maps& T, const DrFusedPtrs& g,
-                                            double* sm, const double* tabs, const unsigned long long* codesrc, const long long codestride,
+template <int RES, int NIT, int TX, int TY, bool BND, int Q>
+__device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, const DrTb2Maps& T, const DrTb2Out& g,
+                                            double* sm, const double* tab, const unsigned long long* codesrc, const long long codestride,
                                             unsigned long long* bars, const int s, const int t, const int k,
                                             const int kb, const int ke, const int i, const int j, const int x0, const int y0,
                                             const bool producer, const bool in1, const bool row2, const bool in2,
@@ -178,9 +226,9 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
                                             unsigned long long& code2, double& rmax, bool& rnan) {
     using Cfg = DrTb2Cfg<TX, TY>;
     constexpr int PL = Cfg::PL;
+    constexpr int PAR = Q & 1;
     const int nx = L.nx, ny = L.ny, nz = L.nz;
     const long long sz = L.sz;
-    const double ih = P.inv_h, c2t = P.c2t;
     const int ke1 = ke + (NIT == 2 ? 1 : 0);                  // one past the last first-iteration layer
     const int k2 = k - 2;
     const bool act1 = k < ke1;                                // uniform over the CTA
@@ -192,36 +240,37 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
     const unsigned long long c2 = code2;                      // layer k-2
 
     // ================= phase alpha =================
-    DrStress6 m2;                                             // second-iteration stresses (own node)
-    double u2x = 0.0, u2y = 0.0, u2z = 0.0;                   // first-iteration velocities of layer k-2 (own node)
+    DrStress6 r2;                                             // second-iteration stresses, own node (TB2_REREAD 0)
+    r2.sxx = r2.syy = r2.szz = r2.txy = r2.txz = r2.tyz = 0.0;
     if (act2) {
         DrStress6 o;
         o.sxx = X1p[Y_SXX * PL]; o.syy = X1p[Y_SYY * PL]; o.szz = X1p[Y_SZZ * PL];
         o.txy = X1p[Y_TXY * PL]; o.txz = X1p[Y_TXZ * PL]; o.tyz = X1p[Y_TYZ * PL];
-        u2x = V1c[0 * PL]; u2y = V1c[1 * PL]; u2z = V1c[2 * PL];
-        m2 = dr_tb2_stress<BND>(P, nx, ny, nz, i, j, k2,
-                                tabs[TB2_TAB_K + (int)(c2 & 255u)], tabs[TB2_TAB_G + (int)(c2 & 255u)],
-                                tabs[TB2_TAB_E + (int)((c2 >> 8) & 255u)], tabs[TB2_TAB_E + (int)((c2 >> 16) & 255u)], tabs[TB2_TAB_E + (int)((c2 >> 24) & 255u)],
-                                u2x, u2y, u2z, V1c[0 * PL + 1], V1c[1 * PL + TX], V1c[0 * PL - TX], V1c[1 * PL - 1],
+        const DrStress6 m2 = dr_tb2_stress<BND>(P, nx, ny, nz, i, j, k2,
+                                dr_tab_at(tab + TB2_S_LAM, dr_code_off(c2, 0)), dr_tab_at(tab + TB2_S_G2, dr_code_off(c2, 0)),
+                                dr_tab_at(tab + TB2_S_ES, dr_code_off(c2, 1)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c2, 2)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c2, 3)),
+                                V1c[0 * PL], V1c[1 * PL], V1c[2 * PL], V1c[0 * PL + 1], V1c[1 * PL + TX], V1c[0 * PL - TX], V1c[1 * PL - 1],
                                 V1n[0 * PL], V1n[1 * PL], V1n[2 * PL], V1n[2 * PL - 1], V1n[2 * PL - TX], o);
         X2p[Z_SXX * PL] = m2.sxx; X2p[Z_SYY * PL] = m2.syy; X2p[Z_TXY * PL] = m2.txy;
         X2p[Z_TXZ * PL] = m2.txz; X2p[Z_TYZ * PL] = m2.tyz;
         gn.txz = m2.txz; gn.tyz = m2.tyz; gn.szz = m2.szz;
+        if (!TB2_REREAD) r2 = m2;
     }
     DrStress6 m1;                                             // first-iteration stresses (own node)
     double vxc = 0.0, vyc = 0.0, vzc = 0.0;
     unsigned long long c1 = 0ull;
     if (act1) {
-        const double* Ac = sm + Cfg::RING_A + (t & 3) * (Cfg::NA * PL) + s;            // layer k
-        const double* An = sm + Cfg::RING_A + ((t + 1) & 3) * (Cfg::NA * PL) + s;      // layer k+1
-        const double* Bs = sm + Cfg::RING_B + (t % 3) * (Cfg::NB * PL) + s;            // set k+1
+        const int qa = TB2_UNROLL4 ? Q : (t & 3);
+        const double* Ac = sm + Cfg::RING_A + qa * (Cfg::NA * PL) + s;                 // layer k
+        const double* An = sm + Cfg::RING_A + ((qa + 1) & 3) * (Cfg::NA * PL) + s;     // layer k+1
+        const double* Bs = sm + Cfg::RING_B + PAR * (Cfg::NB * PL) + s;                // old stresses of this step
         c1 = *reinterpret_cast<const unsigned long long*>(Ac + 3 * PL);
         vxc = Ac[0 * PL]; vyc = Ac[1 * PL]; vzc = Ac[2 * PL];
         DrStress6 o;
         o.sxx = Bs[0 * PL]; o.syy = Bs[1 * PL]; o.szz = Bs[2 * PL]; o.txy = Bs[3 * PL]; o.txz = Bs[4 * PL]; o.tyz = Bs[5 * PL];
         m1 = dr_tb2_stress<BND>(P, nx, ny, nz, i, j, k,
-                                tabs[TB2_TAB_K + (int)(c1 & 255u)], tabs[TB2_TAB_G + (int)(c1 & 255u)],
-                                tabs[TB2_TAB_E + (int)((c1 >> 8) & 255u)], tabs[TB2_TAB_E + (int)((c1 >> 16) & 255u)], tabs[TB2_TAB_E + (int)((c1 >> 24) & 255u)],
+                                dr_tab_at(tab + TB2_S_LAM, dr_code_off(c1, 0)), dr_tab_at(tab + TB2_S_G2, dr_code_off(c1, 0)),
+                                dr_tab_at(tab + TB2_S_ES, dr_code_off(c1, 1)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c1, 2)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c1, 3)),
                                 vxc, vyc, vzc, Ac[0 * PL + 1], Ac[1 * PL + TX], Ac[0 * PL - TX], Ac[1 * PL - 1],
                                 An[0 * PL], An[1 * PL], An[2 * PL], An[2 * PL - 1], An[2 * PL - TX], o);
         // X1p held layer k-2 (read above by this same thread): now layer k
@@ -233,45 +282,43 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
     }
     __syncthreads();
 
-    // ---- every thread is done with ring-A layer k and ring-B set k+1: refill their slots with batch t+4
-    if (producer && k + 4 <= ke1) {
-        const int b = t + 4, m = k + 4;
-        unsigned long long* bar = bars + (b & 3);
-        double* da = sm + Cfg::RING_A + (b & 3) * (Cfg::NA * PL);
-        double* db = sm + Cfg::RING_B + ((b - 1) % 3) * (Cfg::NB * PL);
-        dr_tb2_issue_batch<TX, TY>(T, bar, da, db, codesrc, codestride, x0, y0, m, true);
-    }
-    // ---- the batch of the next step (issued two steps ago)
-    if (k + 2 <= ke1) dr_mbar_wait(bars + ((t + 2) & 3), ((t + 2) >> 2) & 1);
+    // ---- every thread is done with ring-A layer k-1 (since the previous step) and with this step's ring-B set: their
+    // slots take group t+2 = layer k+3 and the stress set of step t+2, one and a half steps ahead of need
+    if (producer && k + 2 < ke1)
+        dr_tb2_issue_group<TX, TY>(T, bars, sm, codesrc, codestride, x0, y0, t + 2, k + 3);
+    // ---- the group of the next step (issued one step ago)
+    if (k + 1 < ke1) dr_mbar_wait(bars + (((TB2_UNROLL4 ? Q : t) + 2) & 3), ((t + 2) >> 2) & 1);
 
     // ================= phase beta =================
     if (act2 && row2) {
         const double* Z = X2p;
         gn.txz_r = Z[Z_TXZ * PL + 1]; gn.tyz_u = Z[Z_TYZ * PL + TX];       // +x / +y neighbours on face k2+1, for the next step
         if (in2 && k2 >= kb) {
-            const long long o = sz * k2;
+            // own second-iteration stresses come back from the exchange planes (not held in registers across the barrier)
+            const double msxx = TB2_REREAD ? Z[Z_SXX * PL] : r2.sxx, msyy = TB2_REREAD ? Z[Z_SYY * PL] : r2.syy, mtxy = TB2_REREAD ? Z[Z_TXY * PL] : r2.txy;
+            double* const po = g.col + sz * k2;
             const bool ck = k2 < nz;
             const bool ci = !BND || i < nx, cj = !BND || j < ny;
             if (ck) {
                 if (cj) {                           // v_x at (i, j+1/2, k2+1/2)
-                    const double Fx = ((m2.sxx - Z[Z_SXX * PL - 1]) + (Z[Z_TXY * PL + TX] - m2.txy) + (m2.txz - gc.txz)) * ih;
-                    g.o_vx[o] = dr_tb2_vel<RES>(u2x, Fx, tabs[TB2_TAB_R + (int)((c2 >> 32) & 255u)], c2t, rmax, rnan);
-                    g.o_txz[o] = gc.txz;
+                    const double Fx = (msxx - Z[Z_SXX * PL - 1]) + (Z[Z_TXY * PL + TX] - mtxy) + (gn.txz - gc.txz);
+                    po[F_VX * g.fs] = dr_tb2_vel<RES>(V1c[0 * PL], Fx, tab, dr_code_off(c2, 4), rmax, rnan);
+                    po[F_TXZ * g.fs] = gc.txz;
                 }
                 if (ci) {                           // v_y at (i+1/2, j, k2+1/2)
-                    const double Fy = ((Z[Z_TXY * PL + 1] - m2.txy) + (m2.syy - Z[Z_SYY * PL - TX]) + (m2.tyz - gc.tyz)) * ih;
-                    g.o_vy[o] = dr_tb2_vel<RES>(u2y, Fy, tabs[TB2_TAB_R + (int)((c2 >> 40) & 255u)], c2t, rmax, rnan);
-                    g.o_tyz[o] = gc.tyz;
+                    const double Fy = (Z[Z_TXY * PL + 1] - mtxy) + (msyy - Z[Z_SYY * PL - TX]) + (gn.tyz - gc.tyz);
+                    po[F_VY * g.fs] = dr_tb2_vel<RES>(V1c[1 * PL], Fy, tab, dr_code_off(c2, 5), rmax, rnan);
+                    po[F_TYZ * g.fs] = gc.tyz;
                 }
-                g.o_txy[o] = m2.txy;
-                if (ci && cj) { g.o_sxx[o] = m2.sxx; g.o_syy[o] = m2.syy; g.o_szz[o] = m2.szz; }
+                po[F_TXY * g.fs] = mtxy;
+                if (ci && cj) { po[F_SXX * g.fs] = msxx; po[F_SYY * g.fs] = msyy; po[F_SZZ * g.fs] = gn.szz; }
             } else {                                // k2 == nz: only the top faces
-                if (cj) g.o_txz[o] = gc.txz;
-                if (ci) g.o_tyz[o] = gc.tyz;
+                if (cj) po[F_TXZ * g.fs] = gc.txz;
+                if (ci) po[F_TYZ * g.fs] = gc.tyz;
             }
             if (ci && cj) {                         // v_z at (i+1/2, j+1/2, k2)
-                const double Fz = ((gc.txz_r - gc.txz) + (gc.tyz_u - gc.tyz) + (m2.szz - gc.szz)) * ih;
-                g.o_vz[o] = dr_tb2_vel<RES>(u2z, Fz, tabs[TB2_TAB_R + (int)((c2 >> 48) & 255u)], c2t, rmax, rnan);
+                const double Fz = (gc.txz_r - gc.txz) + (gc.tyz_u - gc.tyz) + (gn.szz - gc.szz);
+                po[F_VZ * g.fs] = dr_tb2_vel<RES>(V1c[2 * PL], Fz, tab, dr_code_off(c2, 6), rmax, rnan);
             }
         }
     }
@@ -281,27 +328,27 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
         double r1 = 0.0; bool n1 = false;                    // the first iteration of a pair is never a check iteration
         if (in1) {
             fn.txz_r = Y[Y_TXZ * PL + 1]; fn.tyz_u = Y[Y_TYZ * PL + TX];
-            const double Fx = ((m1.sxx - Y[Y_SXX * PL - 1]) + (Y[Y_TXY * PL + TX] - m1.txy) + (m1.txz - fc.txz)) * ih;
-            const double Fy = ((Y[Y_TXY * PL + 1] - m1.txy) + (m1.syy - Y[Y_SYY * PL - TX]) + (m1.tyz - fc.tyz)) * ih;
-            const double Fz = ((fc.txz_r - fc.txz) + (fc.tyz_u - fc.tyz) + (m1.szz - fc.szz)) * ih;
+            const double Fx = (m1.sxx - Y[Y_SXX * PL - 1]) + (Y[Y_TXY * PL + TX] - m1.txy) + (m1.txz - fc.txz);
+            const double Fy = (Y[Y_TXY * PL + 1] - m1.txy) + (m1.syy - Y[Y_SYY * PL - TX]) + (m1.tyz - fc.tyz);
+            const double Fz = (fc.txz_r - fc.txz) + (fc.tyz_u - fc.tyz) + (m1.szz - fc.szz);
             if (NIT == 2) {
-                nvx = dr_tb2_vel<0>(vxc, Fx, tabs[TB2_TAB_R + (int)((c1 >> 32) & 255u)], c2t, r1, n1);
-                nvy = dr_tb2_vel<0>(vyc, Fy, tabs[TB2_TAB_R + (int)((c1 >> 40) & 255u)], c2t, r1, n1);
-                nvz = dr_tb2_vel<0>(vzc, Fz, tabs[TB2_TAB_R + (int)((c1 >> 48) & 255u)], c2t, r1, n1);
+                nvx = dr_tb2_vel<0>(vxc, Fx, tab, dr_code_off(c1, 4), r1, n1);
+                nvy = dr_tb2_vel<0>(vyc, Fy, tab, dr_code_off(c1, 5), r1, n1);
+                nvz = dr_tb2_vel<0>(vzc, Fz, tab, dr_code_off(c1, 6), r1, n1);
             } else if (row2 && in2 && k >= kb) {    // NIT == 1: a plain one-iteration sweep on the same geometry
-                const long long o = sz * k;
+                double* const po = g.col + sz * k;
                 const bool ck = k < nz;
                 const bool ci = !BND || i < nx, cj = !BND || j < ny;
                 if (ck) {
-                    if (cj) { g.o_vx[o] = dr_tb2_vel<RES>(vxc, Fx, tabs[TB2_TAB_R + (int)((c1 >> 32) & 255u)], c2t, rmax, rnan); g.o_txz[o] = fc.txz; }
-                    if (ci) { g.o_vy[o] = dr_tb2_vel<RES>(vyc, Fy, tabs[TB2_TAB_R + (int)((c1 >> 40) & 255u)], c2t, rmax, rnan); g.o_tyz[o] = fc.tyz; }
-                    g.o_txy[o] = m1.txy;
-                    if (ci && cj) { g.o_sxx[o] = m1.sxx; g.o_syy[o] = m1.syy; g.o_szz[o] = m1.szz; }
+                    if (cj) { po[F_VX * g.fs] = dr_tb2_vel<RES>(vxc, Fx, tab, dr_code_off(c1, 4), rmax, rnan); po[F_TXZ * g.fs] = fc.txz; }
+                    if (ci) { po[F_VY * g.fs] = dr_tb2_vel<RES>(vyc, Fy, tab, dr_code_off(c1, 5), rmax, rnan); po[F_TYZ * g.fs] = fc.tyz; }
+                    po[F_TXY * g.fs] = m1.txy;
+                    if (ci && cj) { po[F_SXX * g.fs] = m1.sxx; po[F_SYY * g.fs] = m1.syy; po[F_SZZ * g.fs] = m1.szz; }
                 } else {
-                    if (cj) g.o_txz[o] = fc.txz;
-                    if (ci) g.o_tyz[o] = fc.tyz;
+                    if (cj) po[F_TXZ * g.fs] = fc.txz;
+                    if (ci) po[F_TYZ * g.fs] = fc.tyz;
                 }
-                if (ci && cj) g.o_vz[o] = dr_tb2_vel<RES>(vzc, Fz, tabs[TB2_TAB_R + (int)((c1 >> 48) & 255u)], c2t, rmax, rnan);
+                if (ci && cj) po[F_VZ * g.fs] = dr_tb2_vel<RES>(vzc, Fz, tab, dr_code_off(c1, 6), rmax, rnan);
             }
         }
         if (NIT == 2) { V1c[0 * PL] = nvx; V1c[1 * PL] = nvy; V1c[2 * PL] = nvz; }   // layer k replaces layer k-2 (read above)
@@ -310,8 +357,8 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
 }
 
 template <int RES, int NIT, int TX, int TY, bool BND>
-__device__ __forceinline__ void dr_tb2_march(const DrLayout& L, const DrPT& P, const DrTb2Maps& T, const DrFusedPtrs& g,
-                                             double* sm, const double* tabs, const unsigned long long* codesrc, const long long codestride,
+__device__ __forceinline__ void dr_tb2_march(const DrLayout& L, const DrPT& P, const DrTb2Maps& T, const DrTb2Out& g,
+                                             double* sm, const double* tab, const unsigned long long* codesrc, const long long codestride,
                                              unsigned long long* bars, const int s, const int kb, const int ke,
                                              const int i, const int j, const int x0, const int y0,
                                              const bool producer, const bool in1, const bool row2, const bool in2, double& rmax, bool& rnan) {
@@ -321,36 +368,61 @@ __device__ __forceinline__ void dr_tb2_march(const DrLayout& L, const DrPT& P, c
     unsigned long long ca = 0ull, cb = 0ull;
     const int klast = ke + (NIT == 2 ? 1 : -1);               // last step: second iteration of layer ke-1
     int k = kb - 2;
-    for (int t = 0; k <= klast; t += 2, k += 2) {
-        dr_tb2_step<RES, NIT, TX, TY, BND, 0>(L, P, T, g, sm, tabs, codesrc, codestride, bars, s, t, k, kb, ke, i, j, x0, y0, producer, in1, row2, in2, fa, fb, ga, gb, ca, rmax, rnan);
-        if (k + 1 <= klast)
-            dr_tb2_step<RES, NIT, TX, TY, BND, 1>(L, P, T, g, sm, tabs, codesrc, codestride, bars, s, t + 1, k + 1, kb, ke, i, j, x0, y0, producer, in1, row2, in2, fb, fa, gb, ga, cb, rmax, rnan);
+#define DR_TB2_STEP(Q_, FC, FN, GC, GN, CC) \
+    dr_tb2_step<RES, NIT, TX, TY, BND, Q_>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, t + Q_, k + Q_, kb, ke, i, j, x0, y0, producer, in1, row2, in2, FC, FN, GC, GN, CC, rmax, rnan)
+#if TB2_UNROLL4
+    for (int t = 0; k <= klast; t += 4, k += 4) {
+        DR_TB2_STEP(0, fa, fb, ga, gb, ca);
+        if (k + 1 <= klast) DR_TB2_STEP(1, fb, fa, gb, ga, cb);
+        if (k + 2 <= klast) DR_TB2_STEP(2, fa, fb, ga, gb, ca);
+        if (k + 3 <= klast) DR_TB2_STEP(3, fb, fa, gb, ga, cb);
     }
+#else
+    for (int t = 0; k <= klast; t += 2, k += 2) {
+        DR_TB2_STEP(0, fa, fb, ga, gb, ca);
+        if (k + 1 <= klast) DR_TB2_STEP(1, fb, fa, gb, ga, cb);
+    }
+#endif
+#undef DR_TB2_STEP
 }
 
 // NIT = 2: two PT iterations per launch (RES: the residual max-norm of the SECOND one); NIT = 1: one iteration on the same
 // geometry and tables (kept for A/B checks of the coded path against k_pt_tma).
 template <int RES, int NIT, int TX, int TY>
 __global__ void __launch_bounds__(TX * TY, 1)
-k_pt_tb2(const __grid_constant__ DrTb2Maps T, DrLayout L, DrPT P, DrFields B, int lz, unsigned long long* res_bits) {
+k_pt_tb2(const __grid_constant__ DrTb2Batch TB, DrLayout L, int lz) {
     extern __shared__ __align__(1024) double sm[];
     __shared__ __align__(8) unsigned long long bars[4];
-    __shared__ double tabs[TB2_TAB_N];
+    __shared__ double tab[RES ? 1280 : 1024];
     using Cfg = DrTb2Cfg<TX, TY>;
     constexpr int PL = Cfg::PL;
     const int nx = L.nx, ny = L.ny, nz = L.nz;
     const int tx = threadIdx.x, ty = threadIdx.y;
+    const int slot = blockIdx.z / TB.nchunks, chunk = blockIdx.z - slot * TB.nchunks;
+    const DrPT& P = TB.P[slot];
+    DrTb2Maps T;
+    T.m = TB.m[slot]; T.l2_hint = TB.l2_hint;
     // node of thread (0,0): ib is odd so that the TMA box starts on an even element (16-byte aligned, DR_OX is odd)
     const int ib = blockIdx.x * (TX - 4) - 3, jb = blockIdx.y * (TY - 4) - 2;
     const int i = ib + tx, j = jb + ty;
-    const int kb = blockIdx.z * lz;
+    const int kb = chunk * lz;
     const int ke = min(kb + lz, nz + 1);
-    const int ke1 = ke + (NIT == 2 ? 1 : 0);
     const int x0 = DR_OX + ib, y0 = jb + 1;                  // box origin in padded-field coordinates (z = layer + 1)
-    const long long codestride = (long long)T.gx * T.gy * PL;
-    const unsigned long long* codesrc = T.codes + ((long long)blockIdx.y * T.gx + blockIdx.x) * PL;
+    const long long codestride = (long long)TB.gx * TB.gy * PL;
+    const unsigned long long* codesrc = TB.codes + ((long long)blockIdx.y * TB.gx + blockIdx.x) * PL;
     const int s = ty * TX + tx;
-    for (int e = s; e < TB2_TAB_N; e += TX * TY) tabs[e] = T.tabs[e];
+    // derived tables (see TB2_S_*): the products that do not change from one iteration to the next
+    {
+        const double thh = P.theta * P.inv_h, cvh = P.c2t * P.inv_h;
+        for (int e = s; e < 256; e += TX * TY) {
+            const double Kv = TB.tabs[TB2_TAB_K + e], Gv = TB.tabs[TB2_TAB_G + e], Rv = TB.tabs[TB2_TAB_R + e];
+            tab[TB2_S_LAM + e] = fma(-(2.0 / 3.0), Gv, Kv);
+            tab[TB2_S_G2 + e] = 2.0 * Gv;
+            tab[TB2_S_ES + e] = thh * TB.tabs[TB2_TAB_E + e];
+            tab[TB2_S_CV + e] = cvh * Rv;
+            if (RES) tab[TB2_S_RH + e] = Rv;
+        }
+    }
     const bool producer = (tx == 0 && ty == 0);
     const bool in1 = tx >= 1 && tx <= TX - 2 && ty >= 1 && ty <= TY - 2;
     const bool row2 = ty >= 2 && ty <= TY - 3;
@@ -361,39 +433,31 @@ k_pt_tb2(const __grid_constant__ DrTb2Maps T, DrLayout L, DrPT P, DrFields B, in
         for (int b = 0; b < 4; ++b) dr_mbar_init(bars + b, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        // prologue: batch 0 = layer kb-2 (ring A only), batches 1..3 = layers kb-1 .. kb+1 with their B sets
-#pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            const int m = kb - 2 + b;
-            if (m <= ke1) {
-                double* da = sm + Cfg::RING_A + b * (Cfg::NA * PL);
-                double* db = sm + Cfg::RING_B + (b >= 1 ? b - 1 : 0) * (Cfg::NB * PL);
-                dr_tb2_issue_batch<TX, TY>(T, bars + b, da, db, codesrc, codestride, x0, y0, m, b >= 1);
-            }
-        }
+        // prologue: group -1 = layer kb-2, groups 0 and 1 = layers kb-1, kb with the stress sets of steps 0 and 1
+        dr_tb2_issue_group<TX, TY>(T, bars, sm, codesrc, codestride, x0, y0, -1, kb - 2);
+        dr_tb2_issue_group<TX, TY>(T, bars, sm, codesrc, codestride, x0, y0, 0, kb - 1);
+        dr_tb2_issue_group<TX, TY>(T, bars, sm, codesrc, codestride, x0, y0, 1, kb);
     }
     __syncthreads();                                          // barrier init and tables visible
     dr_mbar_wait(bars + 0, 0);
     dr_mbar_wait(bars + 1, 0);
 
-    const long long qcol = L.origin + min(max(i, 0), nx + 1) + L.sy * min(max(j, 0), ny + 1);
-    DrFusedPtrs g;
-    g.o_vx = B.f[F_VX] + qcol; g.o_vy = B.f[F_VY] + qcol; g.o_vz = B.f[F_VZ] + qcol;
-    g.o_sxx = B.f[F_SXX] + qcol; g.o_syy = B.f[F_SYY] + qcol; g.o_szz = B.f[F_SZZ] + qcol;
-    g.o_tyz = B.f[F_TYZ] + qcol; g.o_txz = B.f[F_TXZ] + qcol; g.o_txy = B.f[F_TXY] + qcol;
+    DrTb2Out g;
+    g.col = TB.out[slot] + (L.origin + min(max(i, 0), nx + 1) + L.sy * min(max(j, 0), ny + 1));
+    g.fs = TB.fs;
     double rmax = 0.0;
     bool rnan = false;
     // extended tile free of boundary nodes?
     const bool interior = ib >= 1 && ib + TX - 1 <= nx - 1 && jb >= 1 && jb + TY - 1 <= ny - 1;
-    if (interior) dr_tb2_march<RES, NIT, TX, TY, false>(L, P, T, g, sm, tabs, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row2, in2, rmax, rnan);
-    else          dr_tb2_march<RES, NIT, TX, TY, true>(L, P, T, g, sm, tabs, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row2, in2, rmax, rnan);
+    if (interior) dr_tb2_march<RES, NIT, TX, TY, false>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row2, in2, rmax, rnan);
+    else          dr_tb2_march<RES, NIT, TX, TY, true>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row2, in2, rmax, rnan);
 
     if (RES) {
         __shared__ unsigned long long smr[32];
-        unsigned long long b = rnan ? 0x7ff8000000000000ull : (unsigned long long)__double_as_longlong(rmax * P.res_scale);
+        unsigned long long b = rnan ? 0x7ff8000000000000ull : (unsigned long long)__double_as_longlong(rmax * (P.inv_h * P.res_scale));
         __syncthreads();
         b = dr_block_max_bits(b, smr);
-        if (tx == 0 && ty == 0 && b != 0ull) atomicMax(res_bits, b);
+        if (tx == 0 && ty == 0 && b != 0ull) atomicMax(TB.res[slot], b);
     }
 }
 

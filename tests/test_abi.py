@@ -37,8 +37,8 @@ def test_workspace_bytes_host_logic(libdr):
     b32 = binding.workspace_bytes(32, 32, 32)
     # 22 padded boxes of PX x 35 x 35 doubles (+ small scratch); PX = 17 + 34 rounded up to 64, +16 off the 512 B pitch
     # + tile-blocked uint8 phase ids: 2 x 3 tiles x 35 layers x 512 B
-    # + stencil codes of the two-iteration kernel: 2 x 4 tiles (28 x 10 owned nodes of 32 x 14) x 37 layers x 448 x 8 B
-    ids = 2 * 3 * 35 * 512 + 2 * 4 * 37 * 448 * 8
+    # + stencil codes of the two-iteration kernel: 2 x 3 tiles (28 x 12 owned nodes of 32 x 16) x 37 layers x 512 x 8 B
+    ids = 2 * 3 * 35 * 512 + 2 * 3 * 37 * 512 * 8
     assert 22 * 80 * 35 * 35 * 8 + ids <= b32 <= 22 * 80 * 35 * 35 * 8 + ids + 22 * 256 + 131072
     assert binding.workspace_bytes(703, 703, 703) < 72e9          # config 5 fits one B200 (180 GB)
 

@@ -158,6 +158,10 @@ def test_cfg4_479_fields_20_iterations_and_which_side_carries_the_average_error(
         assert gpu_err <= 1e-12, (lc, gpu_err, ora_err)
         assert ora_err <= 1e-9, (lc, ora_err)
         s.close(); del s, o
+    # the one-sweep TMA kernel (odd leftovers, uncoded images) at the same size and launch configuration
+    errs, ro, rs, _, _ = run_pair(oracle_mod, gpu, K, G, 4, 1e-4, 5, kernel=0)
+    assert max(errs) <= FIELD_TOL, errs
+    assert abs(ro - rs) <= 1e-9 * ro
 
 
 def test_cfg5_703_fields_20_iterations(oracle_mod, gpu):

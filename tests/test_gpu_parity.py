@@ -52,7 +52,7 @@ def run_pair(oracle_mod, gpu, K, G, lc, eps0, niter, h=1.0, **params):
     return errs, ro, rs, ao, as_
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("lc", range(6))
 def test_fields_config1_sphere_100_iterations(oracle_mod, gpu, kernel, lc):
     K, G, _ = inputs.config1_sphere()
@@ -73,7 +73,7 @@ def test_fields_ragged_noncubic_random_moduli(oracle_mod, gpu, kernel, shape, h)
         assert abs(ro - rs) <= 1e-9 * ro
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4])
 def test_fields_void_and_fluid_cells(oracle_mod, gpu, kernel):
     """degenerate moduli: exact void (K=G=0), fluid (G=0), 1e-6 contrast"""
     K, G, m = inputs.random_two_phase((40, 33, 20), frac=0.3, seed=4, matrix=(37.0, 44.0), incl=(2.2, 0.0))
@@ -85,7 +85,7 @@ def test_fields_void_and_fluid_cells(oracle_mod, gpu, kernel):
         assert np.isfinite(rs) and abs(ro - rs) <= 1e-9 * ro
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("params", [dict(bc_mode=1), dict(gavg=1), dict(cfl=0.5, st_factor=0.7), dict(void_rel=1e-5)])
 def test_fields_parameter_variants(oracle_mod, gpu, kernel, params):
     K, G, _ = inputs.config1_sphere(n=24, r=4.0)
@@ -102,7 +102,7 @@ def test_zero_iterations_is_the_initial_field(oracle_mod, gpu):
         assert np.max(np.abs(ao - as_)) <= 1e-13 * np.max(np.abs(ao))
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
 def test_converged_C_config1(oracle_mod, gpu, kernel):
     """cfg 1 to tol 1e-8, same ncheck on both sides -> same iteration counts; C within 1e-6"""
     K, G, _ = inputs.config1_sphere()
@@ -320,7 +320,9 @@ def test_fuzz_random_shapes_and_parameters(oracle_mod, gpu, seed):
     rng = np.random.default_rng(1000 + seed)
     shape, params, lc, eps0, niter, h = _fuzz_case(rng)
     if seed % 2:                                  # every other case: few distinct (K,G) pairs -> phase-id path
-        K, G = _quantised(shape, int(rng.integers(2, 40)), seed)
+        K, G = _quantised(shape, int(rng.integers(2, 40)) if seed % 4 == 1 else int(rng.integers(2, 5)), seed)
+        if params["kernel"] != 1 and params["form"] == 0:
+            params["kernel"] = 3 if seed % 4 == 3 or params["kernel"] == 0 else 4       # coded kernels (fall back when > 256 edge values)
         if rng.uniform() < 0.3:
             params["void_rel"] = 0.1
     else:
