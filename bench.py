@@ -161,6 +161,8 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
+    if args.cpu_threads > 0:
+        os.environ["OMP_NUM_THREADS"] = str(args.cpu_threads)      # before libdro.so (and its OpenMP runtime) is loaded
     K, G, n = make_image(args.workload, args.n)
     sample_n = min(n, args.cpu_sample_n)
     from oracle import dro
@@ -185,6 +187,14 @@ def run_reference(args):
         "e2e": {"value": rate, "unit": "voxel-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
+    if args.time_to_solution:
+        # the oracle's own time to the full 6x6 tensor (all six load cases to `tol`), same crop
+        o2 = dro.Oracle(Kc, Gc, ncheck=args.ncheck)
+        t0 = time.perf_counter()
+        Cc, log = o2.solve_all(args.eps0, args.tol, 100 * m)
+        line["time_to_full_C"] = {"seconds": time.perf_counter() - t0, "tol": args.tol, "grid": [m, m, m],
+                                  "iters": [l[1] for l in log], "status": [l[0] for l in log],
+                                  "C": [[float("%.6f" % v) for v in row] for row in Cc]}
     print(json.dumps(line))
     return 0
 
@@ -207,6 +217,7 @@ def main():
     ap.add_argument("--cpu-sample-n", type=int, default=191)
     ap.add_argument("--cpu-iters", type=int, default=100)
     ap.add_argument("--cpu-iters-per-step", type=int, default=5)
+    ap.add_argument("--cpu-threads", type=int, default=0, help="--impl reference: OMP_NUM_THREADS of the oracle (0 = all host cores)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-iters", type=int, default=50, help="PT iterations per load case in the host-buffer e2e call")
     ap.add_argument("--time-to-solution", action="store_true", help="also solve all six load cases to tol 1e-8")
