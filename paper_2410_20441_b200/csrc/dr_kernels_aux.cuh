@@ -97,11 +97,13 @@ __global__ void k_bc_init(DrLayout L, DrPT P, DrFields F, DrFields F2, int form,
     S.f[F_SXX][q] = sxx; S.f[F_SYY][q] = syy; S.f[F_SZZ][q] = szz;
     double txy = 0, txz = 0, tyz = 0;
     const bool bi = (i == 0 || i == nx), bj = (j == 0 || j == ny), bk = (k == 0 || k == nz);
-    if (ck && (!(bi || bj) || P.ghost_xy))
+    // a load case drives one strain component: the edge means (four divisions each) are only formed where they matter
+    // (mean x 0 is +0 whatever the mean, so skipping it changes no bit)
+    if (gxy != 0.0 && ck && (!(bi || bj) || P.ghost_xy))
         txy = dr_edge_mean<GAVG>(Gp[q - 1 - sy], Gp[q - sy], Gp[q - 1], Gp[q]) * gxy;
-    if (cj && (!(bi || bk) || P.ghost_xz))
+    if (gxz != 0.0 && cj && (!(bi || bk) || P.ghost_xz))
         txz = dr_edge_mean<GAVG>(Gp[q - 1 - sz], Gp[q - sz], Gp[q - 1], Gp[q]) * gxz;
-    if (ci && (!(bj || bk) || P.ghost_yz))
+    if (gyz != 0.0 && ci && (!(bj || bk) || P.ghost_yz))
         tyz = dr_edge_mean<GAVG>(Gp[q - sy - sz], Gp[q - sz], Gp[q - sy], Gp[q]) * gyz;
     S.f[F_TXY][q] = txy; S.f[F_TXZ][q] = txz; S.f[F_TYZ][q] = tyz;
 }
