@@ -8,6 +8,8 @@
 #include <cstdlib>
 #include <string>
 #include <algorithm>
+#include <mutex>
+#include <vector>
 
 #include "../../include/dr.h"
 #include "dr_layout.cuh"
@@ -208,6 +210,52 @@ static bool make_all_tmaps(dr_handle* H) {
     return make_tmap(H, enc, &H->tm_K, H->K) && make_tmap(H, enc, &H->tm_G, H->G);
 }
 
+// page-locked scratch of a handle (64 doubles: residuals and averages read back at a check).  cudaMallocHost / cudaFreeHost
+// cost more than a whole PT iteration on small grids (the free synchronises the device), so blocks are recycled through a
+// process-wide free list and live until the process ends.
+static std::mutex g_pin_mu;
+static std::vector<double*> g_pin_free;
+static double* pinned_acquire() {
+    {
+        std::lock_guard<std::mutex> lk(g_pin_mu);
+        if (!g_pin_free.empty()) { double* p = g_pin_free.back(); g_pin_free.pop_back(); return p; }
+    }
+    double* p = nullptr;
+    if (cudaHostAlloc((void**)&p, 64 * sizeof(double), cudaHostAllocPortable) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return p;
+}
+static void pinned_release(double* p) {
+    if (!p) return;
+    std::lock_guard<std::mutex> lk(g_pin_mu);
+    g_pin_free.push_back(p);
+}
+
+// opt in to the large dynamic shared memory of the fused kernels (all instantiations), once per device and process: the
+// ~30 attribute calls are a visible part of dr_create on small grids
+static cudaError_t set_kernel_attributes(int device) {
+    static bool done[64] = {false};
+    if (device >= 0 && device < 64 && done[device]) return cudaSuccess;
+    const cudaFuncAttribute A = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    const int smem = (int)DrFusedCfg<FUSED_TX, FUSED_TY>::SMEM;
+    cudaError_t e = cudaFuncSetAttribute(k_pt_fused<0, 0, FUSED_TX, FUSED_TY>, A, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<0, 1, FUSED_TX, FUSED_TY>, A, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 0, FUSED_TX, FUSED_TY>, A, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 1, FUSED_TX, FUSED_TY>, A, smem);
+    const int smem_t = (int)DrTmaCfg2<FUSED_TX, FUSED_TY, 0>::SMEM2, smem_p = (int)DrTmaCfg2<FUSED_TX, FUSED_TY, 1>::SMEM2;
+#define DR_SET_TMA_ATTR(G_, R_, F_) if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<G_, R_, F_, 0, FUSED_TX, FUSED_TY>, A, smem_t); \
+                                    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<G_, R_, F_, 1, FUSED_TX, FUSED_TY>, A, smem_p)
+    DR_SET_TMA_ATTR(0, 0, 0); DR_SET_TMA_ATTR(0, 1, 0); DR_SET_TMA_ATTR(1, 0, 0); DR_SET_TMA_ATTR(1, 1, 0);
+    DR_SET_TMA_ATTR(0, 0, 1); DR_SET_TMA_ATTR(0, 1, 1); DR_SET_TMA_ATTR(1, 0, 1); DR_SET_TMA_ATTR(1, 1, 1);
+#undef DR_SET_TMA_ATTR
+    const int smem2 = (int)DrTb2Cfg<TB2_TX, TB2_TY>::SMEM;
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tb2<0, 2, TB2_TX, TB2_TY>, A, smem2);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tb2<1, 2, TB2_TX, TB2_TY>, A, smem2);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tb2<0, 1, TB2_TX, TB2_TY>, A, smem2);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tb2<1, 1, TB2_TX, TB2_TY>, A, smem2);
+    if (e == cudaSuccess && device >= 0 && device < 64) done[device] = true;
+    return e;
+}
+
 extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K, const double* G,
                                void* workspace, size_t workspace_bytes, void* cuda_stream, dr_handle** out) {
     if (!out) return DR_ERR_ARG;
@@ -262,7 +310,8 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
 
     dr_status st = DR_OK;
     do {
-        if (!cuda_ok(H, cudaMallocHost((void**)&H->pinned, 64 * sizeof(double)), "cudaMallocHost")) { st = DR_ERR_CUDA; break; }
+        H->pinned = pinned_acquire();
+        if (!H->pinned) { H->err = "cudaHostAlloc failed"; st = DR_ERR_CUDA; break; }
         if (!cuda_ok(H, cudaEventCreate(&H->e0), "cudaEventCreate") || !cuda_ok(H, cudaEventCreate(&H->e1), "cudaEventCreate")) { st = DR_ERR_CUDA; break; }
         // state fields and moduli boxes start as zeros (halo nodes are never written afterwards)
         if (!cuda_ok(H, cudaMemsetAsync(workspace, 0, H->nsets == 6 ? dr_workspace_bytes_six(nx, ny, nz) : dr_workspace_bytes(nx, ny, nz), H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }
@@ -298,33 +347,11 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
             H->has_pal = !(fl2 & 4u);
         }
         std::memcpy(&H->hmax, &hb, 8);
-        // opt in to the large dynamic shared memory of the fused kernel (all instantiations)
-        const int smem = (int)DrFusedCfg<FUSED_TX, FUSED_TY>::SMEM;
-        cudaError_t e = cudaSuccess;
-        e = cudaFuncSetAttribute(k_pt_fused<0, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<0, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_fused<1, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (!cuda_ok(H, e, "cudaFuncSetAttribute")) { st = DR_ERR_CUDA; break; }
-        const int smem_t = (int)DrTmaCfg2<FUSED_TX, FUSED_TY, 0>::SMEM2, smem_p = (int)DrTmaCfg2<FUSED_TX, FUSED_TY, 1>::SMEM2;
-#define DR_SET_TMA_ATTR(G_, R_, F_) if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<G_, R_, F_, 0, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t); \
-                                    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tma<G_, R_, F_, 1, FUSED_TX, FUSED_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_p)
-        DR_SET_TMA_ATTR(0, 0, 0); DR_SET_TMA_ATTR(0, 1, 0); DR_SET_TMA_ATTR(1, 0, 0); DR_SET_TMA_ATTR(1, 1, 0);
-        DR_SET_TMA_ATTR(0, 0, 1); DR_SET_TMA_ATTR(0, 1, 1); DR_SET_TMA_ATTR(1, 0, 1); DR_SET_TMA_ATTR(1, 1, 1);
-#undef DR_SET_TMA_ATTR
-        if (!cuda_ok(H, e, "cudaFuncSetAttribute(k_pt_tma)")) { st = DR_ERR_CUDA; break; }
-        {
-            const int smem2 = (int)DrTb2Cfg<TB2_TX, TB2_TY>::SMEM;
-            e = cudaFuncSetAttribute(k_pt_tb2<0, 2, TB2_TX, TB2_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tb2<1, 2, TB2_TX, TB2_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tb2<0, 1, TB2_TX, TB2_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pt_tb2<1, 1, TB2_TX, TB2_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
-            if (!cuda_ok(H, e, "cudaFuncSetAttribute(k_pt_tb2)")) { st = DR_ERR_CUDA; break; }
-        }
+        if (!cuda_ok(H, set_kernel_attributes(H->device), "cudaFuncSetAttribute")) { st = DR_ERR_CUDA; break; }
         if (!make_all_tmaps(H)) { st = DR_ERR_CUDA; break; }
     } while (0);
     if (st != DR_OK) {
-        if (H->pinned) cudaFreeHost(H->pinned);
+        pinned_release(H->pinned);
         if (H->e0) cudaEventDestroy(H->e0);
         if (H->e1) cudaEventDestroy(H->e1);
         delete H;
@@ -351,7 +378,8 @@ extern "C" dr_status dr_set_param(dr_handle* H, int id, double v) {
         case DR_FORM:      if (v != 0.0 && v != 1.0) break; H->form = (int)v; H->cfl = H->form ? 0.50 : 0.55; H->have_fields = false; return DR_OK;
         case DR_PALETTE:   if (v != 0.0 && v != 1.0) break; H->use_pal = (int)v; return DR_OK;
         case DR_ZCHUNK:    if (!(v >= 0.0) || v > 8192.0) break;
-                           H->fused_lz = v >= 1.0 ? (int)v : choose_lz(H->L); H->tb2_lz = v >= 1.0 ? (int)v : choose_lz_tb2(H->L); return DR_OK;
+                           H->fused_lz = v >= 1.0 ? (int)v : choose_lz(H->L); H->tb2_lz = v >= 1.0 ? (int)v : choose_lz_tb2(H->L);
+                           H->lz_user = v >= 1.0; return DR_OK;
         case DR_STAG_TOL:  if (!(v >= 0.0)) break; H->stag_tol = v; return DR_OK;
         default: break;
     }
@@ -461,7 +489,10 @@ static void fill_slot(dr_handle* H, DrTb2Batch& TB, int slot, int set, int cur, 
 // launch the coded kernel on the first nslots slots of TB: nit PT iterations per sweep; with_res: residual of the last
 static dr_status launch_coded(dr_handle* H, DrTb2Batch& TB, int nslots, bool with_res, int nit) {
     const DrLayout& L = H->L;
-    const int lz = H->tb2_lz;
+    // a batch of load cases multiplies the CTA count: pick the z chunk that fills whole waves for THIS number of slots
+    // (small grids: 32^3 runs 2-layer chunks alone and 11-layer chunks with six load cases; results do not depend on it)
+    const int lz = (H->lz_user || nslots == 1) ? H->tb2_lz
+                                               : choose_lz_for(tb2_tiles_x(L) * tb2_tiles_y(L) * nslots, L.nz + 1, 4, DR_LZ_MAX_TB2);
     const int nchunks = (L.nz + 1 + lz - 1) / lz;
     dim3 blk(TB2_TX, TB2_TY, 1), grd(tb2_tiles_x(L), tb2_tiles_y(L), nchunks * nslots);
     TB.fs = H->buf[0][1] - H->buf[0][0];
@@ -774,7 +805,6 @@ extern "C" dr_status dr_solve_all(dr_handle* H, double eps0, double tol, int max
     dr_status worst = DR_OK;
     if (!(H->kernel == 3 && coded(H))) {
         // not a stencil-coded image (or another kernel / form chosen): the six solves one after the other on state set 0
-        cudaEvent_t keep = H->e0;
         for (int lc = 0; lc < 6; ++lc) {
             dr_status s = dr_solve(H, lc, eps0, tol, maxiter);
             H->lc_iters[lc] = H->iters; H->lc_res[lc] = H->residual; H->lc_stop[lc] = H->stop_reason;
@@ -782,7 +812,6 @@ extern "C" dr_status dr_solve_all(dr_handle* H, double eps0, double tol, int max
             if (s != DR_OK && s != DR_MAXITER) return s;
             if (s == DR_MAXITER) worst = DR_MAXITER;
         }
-        (void)keep;
         return worst;
     }
     const DrLayout& L = H->L;
@@ -1039,7 +1068,7 @@ extern "C" void dr_destroy(dr_handle* H) {
     if (!H) return;
     DrDeviceGuard dg(H->device);
     cudaStreamSynchronize(H->st);
-    if (H->pinned) cudaFreeHost(H->pinned);
+    pinned_release(H->pinned);
     if (H->e0) cudaEventDestroy(H->e0);
     if (H->e1) cudaEventDestroy(H->e1);
     delete H;

@@ -141,43 +141,53 @@ __device__ __forceinline__ double dr_warp_sum(double v) {
     return v;
 }
 
-// a6: volume averages (Eq. 7; Reading R7).  Each block walks whole x-rows (j,k) of the node box in a
-// fixed order and writes 6 partial sums; k_avg_final adds the partials in a fixed order -> run-to-run
+// a6: volume averages (Eq. 7; Reading R7).  Each warp walks whole x-rows (j,k) of the node box in a
+// fixed order, each block writes 6 partial sums; k_avg_final adds the partials in a fixed order -> run-to-run
 // deterministic.  Normal stresses: plain cell sum; edge shears: trapezoid weights 1/2 on the first/last index.
 #define DR_AVG_BLOCKS 1184      // 8 x 148 SMs
 #define DR_AVG_THREADS 256
-__global__ void __launch_bounds__(DR_AVG_THREADS)
-k_avg_partial(DrLayout L, DrConstFields F, double* __restrict__ partial) {
+// the six partial sums of one block: warp w of block b takes the x-rows (j,k) number 8 b + w, + 8 gridDim.x, ... (a row is
+// 32 lanes wide per step, four steps of loads in flight per lane), then the warps are added in a fixed order
+__device__ __forceinline__ void dr_avg_block(const DrLayout& L, const DrConstFields& F, double* __restrict__ partial) {
     const int nx = L.nx, ny = L.ny, nz = L.nz;
-    const long long rows = (long long)(ny + 1) * (nz + 1);
+    const int rows = (ny + 1) * (nz + 1);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    constexpr int NW = DR_AVG_THREADS / 32;
     double s[6] = {0, 0, 0, 0, 0, 0};
-    for (long long r = blockIdx.x; r < rows; r += gridDim.x) {
-        int j = (int)(r % (ny + 1)), k = (int)(r / (ny + 1));
+    for (int r = blockIdx.x * NW + warp; r < rows; r += gridDim.x * NW) {
+        const int k = r / (ny + 1), j = r - k * (ny + 1);
         const bool cj = j < ny, ck = k < nz;
         const double wj = (j == 0 || j == ny) ? 0.5 : 1.0, wk = (k == 0 || k == nz) ? 0.5 : 1.0;
-        long long q0 = L.origin + L.sy * j + L.sz * k;
-        for (int i = threadIdx.x; i <= nx; i += blockDim.x) {
-            long long q = q0 + i;
+        const double wjk = wj * wk;
+        const long long q0 = L.origin + L.sy * j + L.sz * k;
+#pragma unroll 4
+        for (int i = lane; i <= nx; i += 32) {
+            const long long q = q0 + i;
             const bool ci = i < nx;
             const double wi = (i == 0 || i == nx) ? 0.5 : 1.0;
             if (ci && cj && ck) { s[0] += F.f[F_SXX][q]; s[1] += F.f[F_SYY][q]; s[2] += F.f[F_SZZ][q]; }
-            if (ci) s[3] += wj * wk * F.f[F_TYZ][q];
+            if (ci) s[3] += wjk * F.f[F_TYZ][q];
             if (cj) s[4] += wi * wk * F.f[F_TXZ][q];
             if (ck) s[5] += wi * wj * F.f[F_TXY][q];
         }
     }
-    __shared__ double sm[6][DR_AVG_THREADS / 32];
+    __shared__ double sm[6][NW];
 #pragma unroll
     for (int m = 0; m < 6; ++m) {
         double v = dr_warp_sum(s[m]);
-        if ((threadIdx.x & 31) == 0) sm[m][threadIdx.x >> 5] = v;
+        if (lane == 0) sm[m][warp] = v;
     }
     __syncthreads();
     if (threadIdx.x < 6) {
         double v = 0;
-        for (int w = 0; w < DR_AVG_THREADS / 32; ++w) v += sm[threadIdx.x][w];
+        for (int w = 0; w < NW; ++w) v += sm[threadIdx.x][w];
         partial[(size_t)blockIdx.x * 6 + threadIdx.x] = v;
     }
+}
+
+__global__ void __launch_bounds__(DR_AVG_THREADS)
+k_avg_partial(DrLayout L, DrConstFields F, double* __restrict__ partial) {
+    dr_avg_block(L, F, partial);
 }
 
 // the same two passes for up to six state sets at once (dr_solve_all): blockIdx.y = slot
@@ -185,38 +195,7 @@ struct DrAvgSix { DrConstFields F[6]; };
 
 __global__ void __launch_bounds__(DR_AVG_THREADS)
 k_avg_partial6(DrLayout L, DrAvgSix A, double* __restrict__ partial6) {
-    const DrConstFields& F = A.F[blockIdx.y];
-    double* partial = partial6 + (size_t)blockIdx.y * DR_AVG_BLOCKS * 6;
-    const int nx = L.nx, ny = L.ny, nz = L.nz;
-    const long long rows = (long long)(ny + 1) * (nz + 1);
-    double s[6] = {0, 0, 0, 0, 0, 0};
-    for (long long r = blockIdx.x; r < rows; r += gridDim.x) {
-        int j = (int)(r % (ny + 1)), k = (int)(r / (ny + 1));
-        const bool cj = j < ny, ck = k < nz;
-        const double wj = (j == 0 || j == ny) ? 0.5 : 1.0, wk = (k == 0 || k == nz) ? 0.5 : 1.0;
-        long long q0 = L.origin + L.sy * j + L.sz * k;
-        for (int i = threadIdx.x; i <= nx; i += blockDim.x) {
-            long long q = q0 + i;
-            const bool ci = i < nx;
-            const double wi = (i == 0 || i == nx) ? 0.5 : 1.0;
-            if (ci && cj && ck) { s[0] += F.f[F_SXX][q]; s[1] += F.f[F_SYY][q]; s[2] += F.f[F_SZZ][q]; }
-            if (ci) s[3] += wj * wk * F.f[F_TYZ][q];
-            if (cj) s[4] += wi * wk * F.f[F_TXZ][q];
-            if (ck) s[5] += wi * wj * F.f[F_TXY][q];
-        }
-    }
-    __shared__ double sm[6][DR_AVG_THREADS / 32];
-#pragma unroll
-    for (int m = 0; m < 6; ++m) {
-        double v = dr_warp_sum(s[m]);
-        if ((threadIdx.x & 31) == 0) sm[m][threadIdx.x >> 5] = v;
-    }
-    __syncthreads();
-    if (threadIdx.x < 6) {
-        double v = 0;
-        for (int w = 0; w < DR_AVG_THREADS / 32; ++w) v += sm[threadIdx.x][w];
-        partial[(size_t)blockIdx.x * 6 + threadIdx.x] = v;
-    }
+    dr_avg_block(L, A.F[blockIdx.y], partial6 + (size_t)blockIdx.y * DR_AVG_BLOCKS * 6);
 }
 
 __global__ void __launch_bounds__(256) k_avg_final(const double* __restrict__ partial, int nblocks, double invN, double* out6) {

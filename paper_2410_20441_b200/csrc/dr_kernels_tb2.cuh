@@ -44,6 +44,12 @@
 #ifndef TB2_REREAD
 #define TB2_REREAD 0       // 1: B2 reads its own second-iteration stresses back from the exchange planes; 0: keeps them in registers
 #endif
+#ifndef TB2_SKIPA2
+#define TB2_SKIPA2 1       // 1: the outermost rows of the extended tile skip the second-iteration stress update (nobody reads it)
+#endif
+#ifndef TB2_LG128
+#define TB2_LG128 0        // 1: lambda and 2G of a cell come with one 16-byte table read
+#endif
 #define TB2_KLO 2          // coded layers below layer 0 (layers -2, -1) ...
 #define TB2_KHI 3          // ... and above layer nz-1 (layers nz, nz+1, nz+2)
 
@@ -55,7 +61,7 @@
 #define TB2_TAB_R 768
 #define TB2_TAB_N 1024
 // what a CTA derives from them once, in shared memory: the products that are the same in every iteration
-//   LAM = K - 2G/3,  G2 = 2G,  ES = (theta/h) E,  CV = (C~^2 h^2 / (theta h)) R,  RH = R (residual launches only)
+//   LAM = K - 2G/3,  G2 = 2G (interleaved, entry e at 2e and 2e+1, when TB2_LG128),  ES = (theta/h) E,  CV = (C~^2 h^2 / (theta h)) R,  RH = R (residual launches only)
 #define TB2_S_LAM 0
 #define TB2_S_G2 256
 #define TB2_S_ES 512
@@ -183,6 +189,16 @@ __device__ __forceinline__ double dr_tab_at(const double* tab, const unsigned of
     return *reinterpret_cast<const double*>(reinterpret_cast<const char*>(tab) + off8);
 }
 
+// lambda = K - 2G/3 and 2G of the cell whose table offset (index x 8) is off8
+__device__ __forceinline__ void dr_tab_lg(const double* tab, const unsigned off8, double& lam, double& g2) {
+#if TB2_LG128
+    const double2 v = *reinterpret_cast<const double2*>(reinterpret_cast<const char*>(tab) + 2u * off8);    // interleaved: one 16-byte read
+    lam = v.x; g2 = v.y;
+#else
+    lam = dr_tab_at(tab + TB2_S_LAM, off8); g2 = dr_tab_at(tab + TB2_S_G2, off8);
+#endif
+}
+
 // TMA group u (u >= 0): what step u needs and no earlier step has brought: ring-A planes of layer m = k_u + 1 (velocities +
 // codes; slot (u+1) & 3) and the old stresses of step u (sxx syy szz txy of layer m-1, txz tyz of face m; ring-B slot u & 1).
 // Group -1 is ring-A layer kb-2 alone.  Completion: mbarrier (u+1) & 3, phase ((u+1) >> 2) & 1.
@@ -221,7 +237,7 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
                                             double* sm, const double* tab, const unsigned long long* codesrc, const long long codestride,
                                             unsigned long long* bars, const int s, const int t, const int k,
                                             const int kb, const int ke, const int i, const int j, const int x0, const int y0,
-                                            const bool producer, const bool in1, const bool row2, const bool in2,
+                                            const bool producer, const bool in1, const bool row1, const bool row2, const bool in2,
                                             const DrFace5& fc, DrFace5& fn, const DrFace5& gc, DrFace5& gn,
                                             unsigned long long& code2, double& rmax, bool& rnan) {
     using Cfg = DrTb2Cfg<TX, TY>;
@@ -242,12 +258,14 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
     // ================= phase alpha =================
     DrStress6 r2;                                             // second-iteration stresses, own node (TB2_REREAD 0)
     r2.sxx = r2.syy = r2.szz = r2.txy = r2.txz = r2.tyz = 0.0;
-    if (act2) {
+    // second-iteration stresses are read by B2 at the inner rows and their +-1 neighbours: rows 1 .. TY-2 (a warp is a row)
+    if (act2 && (!TB2_SKIPA2 || row1)) {
         DrStress6 o;
         o.sxx = X1p[Y_SXX * PL]; o.syy = X1p[Y_SYY * PL]; o.szz = X1p[Y_SZZ * PL];
         o.txy = X1p[Y_TXY * PL]; o.txz = X1p[Y_TXZ * PL]; o.tyz = X1p[Y_TYZ * PL];
-        const DrStress6 m2 = dr_tb2_stress<BND>(P, nx, ny, nz, i, j, k2,
-                                dr_tab_at(tab + TB2_S_LAM, dr_code_off(c2, 0)), dr_tab_at(tab + TB2_S_G2, dr_code_off(c2, 0)),
+        double lam2, g22;
+        dr_tab_lg(tab, dr_code_off(c2, 0), lam2, g22);
+        const DrStress6 m2 = dr_tb2_stress<BND>(P, nx, ny, nz, i, j, k2, lam2, g22,
                                 dr_tab_at(tab + TB2_S_ES, dr_code_off(c2, 1)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c2, 2)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c2, 3)),
                                 V1c[0 * PL], V1c[1 * PL], V1c[2 * PL], V1c[0 * PL + 1], V1c[1 * PL + TX], V1c[0 * PL - TX], V1c[1 * PL - 1],
                                 V1n[0 * PL], V1n[1 * PL], V1n[2 * PL], V1n[2 * PL - 1], V1n[2 * PL - TX], o);
@@ -268,8 +286,9 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
         vxc = Ac[0 * PL]; vyc = Ac[1 * PL]; vzc = Ac[2 * PL];
         DrStress6 o;
         o.sxx = Bs[0 * PL]; o.syy = Bs[1 * PL]; o.szz = Bs[2 * PL]; o.txy = Bs[3 * PL]; o.txz = Bs[4 * PL]; o.tyz = Bs[5 * PL];
-        m1 = dr_tb2_stress<BND>(P, nx, ny, nz, i, j, k,
-                                dr_tab_at(tab + TB2_S_LAM, dr_code_off(c1, 0)), dr_tab_at(tab + TB2_S_G2, dr_code_off(c1, 0)),
+        double lam1, g21;
+        dr_tab_lg(tab, dr_code_off(c1, 0), lam1, g21);
+        m1 = dr_tb2_stress<BND>(P, nx, ny, nz, i, j, k, lam1, g21,
                                 dr_tab_at(tab + TB2_S_ES, dr_code_off(c1, 1)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c1, 2)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c1, 3)),
                                 vxc, vyc, vzc, Ac[0 * PL + 1], Ac[1 * PL + TX], Ac[0 * PL - TX], Ac[1 * PL - 1],
                                 An[0 * PL], An[1 * PL], An[2 * PL], An[2 * PL - 1], An[2 * PL - TX], o);
@@ -361,7 +380,7 @@ __device__ __forceinline__ void dr_tb2_march(const DrLayout& L, const DrPT& P, c
                                              double* sm, const double* tab, const unsigned long long* codesrc, const long long codestride,
                                              unsigned long long* bars, const int s, const int kb, const int ke,
                                              const int i, const int j, const int x0, const int y0,
-                                             const bool producer, const bool in1, const bool row2, const bool in2, double& rmax, bool& rnan) {
+                                             const bool producer, const bool in1, const bool row1, const bool row2, const bool in2, double& rmax, bool& rnan) {
     DrFace5 fa, fb, ga, gb;
     fa.txz = fa.tyz = fa.szz = fa.txz_r = fa.tyz_u = 0.0;
     fb = fa; ga = fa; gb = fa;
@@ -369,7 +388,7 @@ __device__ __forceinline__ void dr_tb2_march(const DrLayout& L, const DrPT& P, c
     const int klast = ke + (NIT == 2 ? 1 : -1);               // last step: second iteration of layer ke-1
     int k = kb - 2;
 #define DR_TB2_STEP(Q_, FC, FN, GC, GN, CC) \
-    dr_tb2_step<RES, NIT, TX, TY, BND, Q_>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, t + Q_, k + Q_, kb, ke, i, j, x0, y0, producer, in1, row2, in2, FC, FN, GC, GN, CC, rmax, rnan)
+    dr_tb2_step<RES, NIT, TX, TY, BND, Q_>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, t + Q_, k + Q_, kb, ke, i, j, x0, y0, producer, in1, row1, row2, in2, FC, FN, GC, GN, CC, rmax, rnan)
 #if TB2_UNROLL4
     for (int t = 0; k <= klast; t += 4, k += 4) {
         DR_TB2_STEP(0, fa, fb, ga, gb, ca);
@@ -393,7 +412,7 @@ __global__ void __launch_bounds__(TX * TY, 1)
 k_pt_tb2(const __grid_constant__ DrTb2Batch TB, DrLayout L, int lz) {
     extern __shared__ __align__(1024) double sm[];
     __shared__ __align__(8) unsigned long long bars[4];
-    __shared__ double tab[RES ? 1280 : 1024];
+    __shared__ __align__(16) double tab[RES ? 1280 : 1024];
     using Cfg = DrTb2Cfg<TX, TY>;
     constexpr int PL = Cfg::PL;
     const int nx = L.nx, ny = L.ny, nz = L.nz;
@@ -416,8 +435,8 @@ k_pt_tb2(const __grid_constant__ DrTb2Batch TB, DrLayout L, int lz) {
         const double thh = P.theta * P.inv_h, cvh = P.c2t * P.inv_h;
         for (int e = s; e < 256; e += TX * TY) {
             const double Kv = TB.tabs[TB2_TAB_K + e], Gv = TB.tabs[TB2_TAB_G + e], Rv = TB.tabs[TB2_TAB_R + e];
-            tab[TB2_S_LAM + e] = fma(-(2.0 / 3.0), Gv, Kv);
-            tab[TB2_S_G2 + e] = 2.0 * Gv;
+            tab[TB2_LG128 ? 2 * e : TB2_S_LAM + e] = fma(-(2.0 / 3.0), Gv, Kv);
+            tab[TB2_LG128 ? 2 * e + 1 : TB2_S_G2 + e] = 2.0 * Gv;
             tab[TB2_S_ES + e] = thh * TB.tabs[TB2_TAB_E + e];
             tab[TB2_S_CV + e] = cvh * Rv;
             if (RES) tab[TB2_S_RH + e] = Rv;
@@ -425,6 +444,7 @@ k_pt_tb2(const __grid_constant__ DrTb2Batch TB, DrLayout L, int lz) {
     }
     const bool producer = (tx == 0 && ty == 0);
     const bool in1 = tx >= 1 && tx <= TX - 2 && ty >= 1 && ty <= TY - 2;
+    const bool row1 = ty >= 1 && ty <= TY - 2;
     const bool row2 = ty >= 2 && ty <= TY - 3;
     const bool in2 = tx >= 2 && tx <= TX - 3 && i >= 0 && i <= nx && j <= ny;
 
@@ -449,8 +469,8 @@ k_pt_tb2(const __grid_constant__ DrTb2Batch TB, DrLayout L, int lz) {
     bool rnan = false;
     // extended tile free of boundary nodes?
     const bool interior = ib >= 1 && ib + TX - 1 <= nx - 1 && jb >= 1 && jb + TY - 1 <= ny - 1;
-    if (interior) dr_tb2_march<RES, NIT, TX, TY, false>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row2, in2, rmax, rnan);
-    else          dr_tb2_march<RES, NIT, TX, TY, true>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row2, in2, rmax, rnan);
+    if (interior) dr_tb2_march<RES, NIT, TX, TY, false>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row1, row2, in2, rmax, rnan);
+    else          dr_tb2_march<RES, NIT, TX, TY, true>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row1, row2, in2, rmax, rnan);
 
     if (RES) {
         __shared__ unsigned long long smr[32];
