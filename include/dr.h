@@ -153,6 +153,15 @@ dr_status dr_iterate(dr_handle* h, int load_case, double eps0, int niter);
  * load cases have been solved.  Not symmetrised. */
 dr_status dr_effective_C(dr_handle* h, double out[36]);
 
+/* The paper's 7th direct test (App. A.3).  load_case 6 of dr_solve / dr_step prescribes the normal displacement
+ * of all three face pairs at once (Dxx = Dyy = Dzz = eps0; tangential components free as in the normal tests).  After load
+ * cases 0, 1, 2 and 6 have been solved on this handle, Eq. 24-29 give the off-diagonal normal components from
+ * sigma_bar_k = <sigma_kk> - C_kk eps_k and eps_bar_k = eps0:  out = (C12, C13, C23), HOST pointer.  The problem is linear,
+ * so these equal the symmetrised off-diagonals of dr_effective_C to solver tolerance (a consistency diagnostic; the six
+ * columns already hold C12, C13, C23).  DR_ERR_STATE until the four load cases exist.  Load case 6 is not part of
+ * dr_effective_C, dr_solve_all or dr_solve_six. */
+dr_status dr_offdiag_direct(dr_handle* h, double out[3]);
+
 /* Volume-averaged stresses of the last solve/step, HOST pointer, Voigt order (Eq. 7). */
 dr_status dr_avg_stress(dr_handle* h, double out[6]);
 

@@ -76,8 +76,8 @@ struct dro_handle {
     /* edge shear moduli (O2), tabulated once per solve from K,G by Ctx::Gxy/Gxz/Gyz */
     std::vector<double> eGxy, eGxz, eGyz;
     /* results */
-    double Ccol[6][6];               /* Ccol[lc][m] = C[m, lc]                      */
-    bool have[6];
+    double Ccol[7][6];               /* Ccol[lc][m] = C[m, lc]; row 6 = <sigma>/eps0 of the triaxial test (App. A.3) */
+    bool have[7];
     double avg[6];
     bool have_avg;
     int iters;
@@ -132,7 +132,9 @@ struct Ctx {
 };
 
 /* Load case -> displacement gradient D (reading R6; P:347-357 A.1, P:365-369 A.2):
- * lc 0,1,2: Dxx,Dyy,Dzz = eps0;  lc 3 (yz): u_y = eps0 z;  lc 4 (xz): u_x = eps0 z;  lc 5 (xy): u_x = eps0 y. */
+ * lc 0,1,2: Dxx,Dyy,Dzz = eps0;  lc 3 (yz): u_y = eps0 z;  lc 4 (xz): u_x = eps0 z;  lc 5 (xy): u_x = eps0 y.
+ * lc 6: the 7th direct test of App. A.3: the normal displacement of all three face pairs is prescribed at
+ * once (Dxx = Dyy = Dzz = eps0), tangential components free as in the normal tests. */
 struct Affine {
     double D[3][3];
     Affine(int lc, double e) {
@@ -144,6 +146,7 @@ struct Affine {
             case 3: D[1][2] = e; break;
             case 4: D[0][2] = e; break;
             case 5: D[0][1] = e; break;
+            case 6: D[0][0] = e; D[1][1] = e; D[2][2] = e; break;
         }
     }
     inline double u(int a, double x, double y, double z) const { return D[a][0] * x + D[a][1] * y + D[a][2] * z; }
@@ -395,7 +398,7 @@ void store_column(dro_handle* H, int lc, double eps0) {
 
 bool bad_solve_args(dro_handle* H, int lc, double eps0) {
     if (!H) return true;
-    if (lc < 0 || lc > 5 || !(eps0 != 0.0) || !std::isfinite(eps0)) { H->err = "bad load case or eps0"; return true; }
+    if (lc < 0 || lc > 6 || !(eps0 != 0.0) || !std::isfinite(eps0)) { H->err = "bad load case or eps0"; return true; }
     return false;
 }
 
@@ -415,7 +418,7 @@ int dro_create(int nx, int ny, int nz, double h, const double* K, const double* 
     H->K0.assign(K, K + N); H->G0.assign(G, G + N);
     H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->form = 0;
     H->stag_tol = 1e-10; H->stop_reason = DRO_STOP_NONE;
-    for (int a = 0; a < 6; ++a) { H->have[a] = false; for (int b = 0; b < 6; ++b) H->Ccol[a][b] = 0.0; }
+    for (int a = 0; a < 7; ++a) { H->have[a] = false; for (int b = 0; b < 6; ++b) H->Ccol[a][b] = 0.0; }
     H->have_avg = false; H->iters = 0; H->residual = 0.0; H->ms = 0.0;
     *out = H;
     return DRO_OK;
@@ -515,6 +518,21 @@ int dro_effective_C(dro_handle* H, double out[36]) {
     if (!H || !out) return DRO_ERR_ARG;
     for (int lc = 0; lc < 6; ++lc) if (!H->have[lc]) { H->err = "not all six load cases solved"; return DRO_ERR_STATE; }
     for (int m = 0; m < 6; ++m) for (int lc = 0; lc < 6; ++lc) out[6 * m + lc] = H->Ccol[lc][m];
+    return DRO_OK;
+}
+
+/* Eq. 24-29: off-diagonal normal components from the 7th (triaxial) test.  With eps_k = eps0 in all three
+ * directions, sigma_bar_k = <sigma_kk> - C_kk eps_k (Eq. 24, C_kk from the direct normal tests lc 0-2) and
+ * eps_bar_k = eps_k (Eq. 25):  out = (C12, C13, C23) of Eq. 27, 28, 29.  Ccol[6] holds <sigma>/eps0 of the triaxial test,
+ * so eps0 cancels: sb_k = Ccol[6][k] - Ccol[k][k] and eb_k = 1. */
+int dro_offdiag_direct(dro_handle* H, double out[3]) {
+    if (!H || !out) return DRO_ERR_ARG;
+    for (int lc : {0, 1, 2, 6}) if (!H->have[lc]) { H->err = "needs load cases 0, 1, 2 and 6"; return DRO_ERR_STATE; }
+    const double sb1 = H->Ccol[6][0] - H->Ccol[0][0], sb2 = H->Ccol[6][1] - H->Ccol[1][1], sb3 = H->Ccol[6][2] - H->Ccol[2][2];
+    const double e1 = 1.0, e2 = 1.0, e3 = 1.0;
+    out[0] = (e1 * sb1 + e2 * sb2 - e3 * sb3) / (2.0 * e1 * e2);     /* Eq. 27 */
+    out[1] = (e1 * sb1 - e2 * sb2 + e3 * sb3) / (2.0 * e1 * e3);     /* Eq. 28 */
+    out[2] = (-e1 * sb1 + e2 * sb2 + e3 * sb3) / (2.0 * e2 * e3);    /* Eq. 29 */
     return DRO_OK;
 }
 

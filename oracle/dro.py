@@ -48,6 +48,7 @@ def lib():
         L.dro_iterate.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_int]
         L.dro_effective_C.argtypes = [C.c_void_p, dp]
         L.dro_avg_stress.argtypes = [C.c_void_p, dp]
+        L.dro_offdiag_direct.argtypes = [C.c_void_p, dp]
         L.dro_info.argtypes = [C.c_void_p, C.POINTER(C.c_int), dp, dp]
         L.dro_field_size.argtypes = [C.c_void_p, C.c_int]
         L.dro_field_size.restype = C.c_size_t
@@ -116,6 +117,12 @@ class Oracle:
     def avg_stress(self):
         out = np.zeros(6)
         self._check(lib().dro_avg_stress(self._h, _dp(out)))
+        return out
+
+    def offdiag_direct(self):
+        """(C12, C13, C23) by Eq. 27-29 from the triaxial test (load case 6) and C11, C22, C33 of load cases 0-2"""
+        out = np.zeros(3)
+        self._check(lib().dro_offdiag_direct(self._h, _dp(out)))
         return out
 
     def info(self):

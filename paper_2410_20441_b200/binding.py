@@ -18,7 +18,7 @@ STOP_NONE, STOP_RESIDUAL, STOP_STAGNATION, STOP_MAXITER = range(4)
 PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK, form=FORM, palette=PALETTE, stag_tol=STAG_TOL)
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
 EXPORTS = ("dr_workspace_bytes", "dr_workspace_bytes_six", "dr_solve_all", "dr_info_lc", "dr_create", "dr_set_param", "dr_solve", "dr_solve_six", "dr_effective_C_six", "dr_step", "dr_iterate",
-           "dr_effective_C", "dr_avg_stress", "dr_info", "dr_get_field", "dr_solve_image_host", "dr_contribution_tensor",
+           "dr_effective_C", "dr_avg_stress", "dr_offdiag_direct", "dr_info", "dr_get_field", "dr_solve_image_host", "dr_contribution_tensor",
            "dr_uses_palette", "dr_active_kernel", "dr_stop_reason", "dr_launch_count", "dr_last_error", "dr_destroy")
 
 _lib = None
@@ -50,6 +50,8 @@ def lib():
         L.dr_iterate.argtypes = [vp, C.c_int, C.c_double, C.c_int]
         L.dr_effective_C.argtypes = [vp, dp]
         L.dr_avg_stress.argtypes = [vp, dp]
+        if hasattr(L, "dr_offdiag_direct"):
+            L.dr_offdiag_direct.argtypes = [vp, dp]
         L.dr_info.argtypes = [vp, C.POINTER(C.c_int), dp, dp]
         L.dr_get_field.argtypes = [vp, C.c_int, vp, C.c_size_t]
         L.dr_solve_image_host.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, vp, vp, vp, vp, C.c_size_t, vp,
@@ -150,6 +152,13 @@ class Solver:
         import numpy as np
         out = np.zeros(6)
         self._check(lib().dr_avg_stress(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def offdiag_direct(self):
+        """dr_offdiag_direct: (C12, C13, C23) by Eq. 27-29 from the triaxial test (load case 6) and load cases 0-2"""
+        import numpy as np
+        out = np.zeros(3)
+        self._check(lib().dr_offdiag_direct(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
         return out
 
     def info(self):

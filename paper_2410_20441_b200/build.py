@@ -25,15 +25,14 @@ def _nvcc():
 
 
 def source_hash():
-    """sha256 (first 16 hex digits) of the CUDA sources and the public header: identifies the kernels a profile under
-    profiles/ was taken with (bench.py emits roofline.traffic only for a matching hash)."""
+    """sha256 (first 16 hex digits) of the CUDA kernel sources (csrc/*.cuh): identifies the kernels a profile under
+    profiles/ was taken with (bench.py emits roofline.traffic only for a matching hash).  The host file dr_api.cu and the
+    public header are left out on purpose: they launch the kernels but do not change what a launch moves."""
     import hashlib
     h = hashlib.sha256()
-    for f in sorted(SOURCES + HEADERS):
+    for f in sorted(HEADERS):
         with open(os.path.join(CSRC, f), "rb") as fh:
             h.update(f.encode() + b"\0" + fh.read())
-    with open(os.path.join(HERE, "..", "include", "dr.h"), "rb") as fh:
-        h.update(b"dr.h\0" + fh.read())
     return h.hexdigest()[:16]
 
 

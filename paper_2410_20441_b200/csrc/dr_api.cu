@@ -58,8 +58,8 @@ struct dr_handle {
     int cur_lc;
     double cur_eps0;
     // results
-    double Ccol[6][6];
-    bool have[6];
+    double Ccol[7][6];          // Ccol[lc][m] = <sigma_m> / eps0 of load case lc; row 6: the triaxial test of App. A.3
+    bool have[7];
     double avg[6];
     bool have_avg;
     int iters;
@@ -304,7 +304,8 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
     H->cfl = 0.55; H->st_factor = 1.0; H->void_rel = 0.0; H->ncheck = 50; H->gavg = 0; H->bc_mode = 0; H->kernel = 3; H->form = 0;
     H->void_applied = 0.0; H->hmax = 0.0;
     H->cur = 0; H->have_fields = false; H->cur_lc = -1; H->cur_eps0 = 0.0;
-    for (int a = 0; a < 6; ++a) { H->have[a] = false; H->avg[a] = 0; for (int b = 0; b < 6; ++b) H->Ccol[a][b] = 0.0; }
+    for (int a = 0; a < 7; ++a) { H->have[a] = false; for (int b = 0; b < 6; ++b) H->Ccol[a][b] = 0.0; }
+    for (int a = 0; a < 6; ++a) H->avg[a] = 0;
     H->have_avg = false; H->iters = 0; H->residual = 0.0; H->ms = 0.0; H->launches = 0;
     H->fused_lz = choose_lz(H->L);
 
@@ -398,7 +399,8 @@ static DrPT make_pt(const dr_handle* H, int lc, double eps0) {
     P.h = H->h; P.inv_h = 1.0 / H->h;
     for (int a = 0; a < 9; ++a) P.D[a] = 0.0;
     static const int slot[6] = {0, 4, 8, 5, 2, 1};                        // Dxx Dyy Dzz Dyz Dxz Dxy
-    P.D[slot[lc]] = eps0;
+    if (lc == 6) { P.D[0] = eps0; P.D[4] = eps0; P.D[8] = eps0; }         // 7th direct test (App. A.3): triaxial
+    else P.D[slot[lc]] = eps0;
     P.Lx = L.nx * H->h; P.Ly = L.ny * H->h; P.Lz = L.nz * H->h;
     P.res_scale = H->h / std::fabs(eps0);
     P.ghost_yz = (H->bc_mode == 1 || lc == 3);
@@ -652,7 +654,7 @@ struct DrStag {
 };
 
 static bool bad_lc(dr_handle* H, int lc, double eps0) {
-    if (lc < 0 || lc > 5 || !(eps0 != 0.0) || !std::isfinite(eps0)) { H->err = "bad load case or eps0"; return true; }
+    if (lc < 0 || lc > 6 || !(eps0 != 0.0) || !std::isfinite(eps0)) { H->err = "bad load case or eps0"; return true; }
     return false;
 }
 
@@ -952,6 +954,19 @@ extern "C" dr_status dr_effective_C(dr_handle* H, double out[36]) {
     if (!H || !out) return DR_ERR_ARG;
     for (int lc = 0; lc < 6; ++lc) if (!H->have[lc]) return fail(H, DR_ERR_STATE, "not all six load cases solved");
     for (int m = 0; m < 6; ++m) for (int lc = 0; lc < 6; ++lc) out[6 * m + lc] = H->Ccol[lc][m];
+    return DR_OK;
+}
+
+// Eq. 24-29: C12, C13, C23 from the 7th (triaxial) direct test, load case 6, and C11, C22, C33 of the normal
+// tests.  Ccol holds <sigma>/eps0, so with eps_bar_k = eps0 (Eq. 25) the strains cancel: sigma_bar_k / eps0 = Ccol[6][k] - C_kk.
+extern "C" dr_status dr_offdiag_direct(dr_handle* H, double out[3]) {
+    if (!H || !out) return DR_ERR_ARG;
+    static const int need[4] = {0, 1, 2, 6};
+    for (int q = 0; q < 4; ++q) if (!H->have[need[q]]) return fail(H, DR_ERR_STATE, "dr_offdiag_direct needs load cases 0, 1, 2 and 6");
+    const double sb1 = H->Ccol[6][0] - H->Ccol[0][0], sb2 = H->Ccol[6][1] - H->Ccol[1][1], sb3 = H->Ccol[6][2] - H->Ccol[2][2];
+    out[0] = 0.5 * (sb1 + sb2 - sb3);      // Eq. 27
+    out[1] = 0.5 * (sb1 - sb2 + sb3);      // Eq. 28
+    out[2] = 0.5 * (-sb1 + sb2 + sb3);     // Eq. 29
     return DR_OK;
 }
 

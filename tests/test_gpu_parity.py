@@ -441,3 +441,28 @@ def test_set_param_discards_fields_built_under_old_parameters(gpu):
     s.step(0, 1e-4, 3)
     s.set_param("ncheck", 7); s.set_param("zchunk", 4); s.set_param("palette", 0); s.set_param("stag_tol", 0.0)
     s.iterate(0, 1e-4, 2)                           # these do not shape the iterate
+
+
+# ------------------------------------------------------------------------------------------------ 7th direct test (App. A.3)
+def test_triaxial_load_case_and_eq27_29_vs_oracle(oracle_mod, gpu):
+    """load case 6 and dr_offdiag_direct (Eq. 24-29): fields after a fixed iteration count and the three
+    off-diagonal components at convergence against the oracle; equal to the symmetrised columns of the six-test C"""
+    K, G = _quantised((26, 22, 30), 3, seed=5)
+    errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, 6, 1e-4, 40)
+    assert max(errs) <= FIELD_TOL, errs
+    assert abs(ro - rs) <= 1e-9 * ro and np.max(np.abs(ao - as_)) <= 1e-10 * np.max(np.abs(ao))
+    s = gpu.Solver(to_dev(K), to_dev(G))
+    o = oracle_mod.Oracle(K, G)
+    with pytest.raises(gpu.DrError) as e:
+        s.offdiag_direct()
+    assert e.value.status == gpu.ERR_STATE
+    for lc in (0, 1, 2, 6):
+        assert s.solve(lc, 1e-4, 1e-9, 20000) == 0 and o.solve(lc, 1e-4, 1e-9, 20000) == 0
+        assert s.info()[0] == o.info()[0]
+    d, do = s.offdiag_direct(), o.offdiag_direct()
+    assert np.max(np.abs(d - do)) <= C_TOL * np.max(np.abs(do)), (d, do)
+    for lc in (3, 4, 5):
+        assert s.solve(lc, 1e-4, 1e-9, 20000) == 0
+    C = s.effective_C()
+    sym = np.array([0.5 * (C[0, 1] + C[1, 0]), 0.5 * (C[0, 2] + C[2, 0]), 0.5 * (C[1, 2] + C[2, 1])])
+    assert np.max(np.abs(d - sym)) <= 1e-6 * C[0, 0]

@@ -276,6 +276,41 @@ def test_P9_paper_eq27_29_offdiagonal_recipe(two_phase):
     assert abs(C23 - 0.5 * (C[1, 2] + C[2, 1])) <= 1e-9 * C[0, 0]
 
 
+def test_P9b_seventh_direct_test_triaxial_load_case(two_phase, oracle_mod):
+    """App. A.3 run as a load case of its own (lc 6: all three normal displacements prescribed at once).
+    Pins: (i) a homogeneous block returns lambda = K - 2G/3 for all three components, in zero iterations; (ii) the
+    problem is linear, so <sigma> of the triaxial solve is the sum of columns 0-2 of the six-test C and Eq. 27-29 (the
+    library routine) agree with the symmetrised off-diagonals of the six-test C; (iii) a two-layer medium, where
+    C12 != C13 = C23, against the Backus averages (the analytic column of the paper's Table 2): a swapped or
+    sign-flipped term in Eq. 27-29 fails here."""
+    Kh = np.full((6, 5, 4), 37.0); Gh = np.full((6, 5, 4), 44.0)
+    o = oracle_mod.Oracle(Kh, Gh, ncheck=1)
+    for lc in (0, 1, 2, 6):
+        assert o.solve(lc, 1e-4, 1e-12, 5) == 0 and o.info()[0] == 1
+    assert np.allclose(o.offdiag_direct(), 37.0 - 2 * 44.0 / 3, rtol=1e-13)
+    K, G, m, C, _ = two_phase
+    o = oracle_mod.Oracle(K, G)
+    for lc in (0, 1, 2, 6):
+        assert o.solve(lc, 1e-4, 1e-9, 20000) == 0
+    tri = o.avg_stress() / 1e-4
+    assert np.max(np.abs(tri[:3] - C[:3, :3].sum(axis=1))) <= 1e-8 * C[0, 0]          # linearity: sum of the normal columns
+    assert np.max(np.abs(tri[3:])) <= 1e-8 * C[0, 0] + np.max(np.abs(C[3:, :3].sum(axis=1)))
+    d = o.offdiag_direct()
+    sym = np.array([0.5 * (C[0, 1] + C[1, 0]), 0.5 * (C[0, 2] + C[2, 0]), 0.5 * (C[1, 2] + C[2, 1])])
+    assert np.max(np.abs(d - sym)) <= 1e-7 * C[0, 0], (d, sym)
+    # layered medium (two layers along z): C12 != C13 = C23, so a swapped equation shows
+    Kl = np.where(np.arange(8)[:, None, None] < 4, 20.0, 60.0) * np.ones((8, 6, 6)); Gl = np.where(np.arange(8)[:, None, None] < 4, 8.0, 30.0) * np.ones((8, 6, 6))
+    o = oracle_mod.Oracle(Kl, Gl)
+    for lc in (0, 1, 2, 6):
+        assert o.solve(lc, 1e-4, 1e-10, 20000) == 0
+    d = o.offdiag_direct()
+    lam = Kl[:, 0, 0] - 2 * Gl[:, 0, 0] / 3; M = Kl[:, 0, 0] + 4 * Gl[:, 0, 0] / 3
+    C13_backus = np.mean(lam / M) / np.mean(1 / M)                                         # Backus average (P:170-183 analytic column)
+    C12_backus = np.mean(lam) - np.mean(lam * lam / M) + np.mean(lam / M) ** 2 / np.mean(1 / M)
+    assert abs(d[1] - C13_backus) <= 1e-6 * C13_backus and abs(d[2] - C13_backus) <= 1e-6 * C13_backus
+    assert abs(d[0] - C12_backus) <= 1e-6 * C12_backus and abs(C12_backus - C13_backus) > 1.0
+
+
 def test_P12_linearity_in_eps0(two_phase):
     K, G, m, C, o = two_phase
     for lc in (1, 4):
@@ -484,7 +519,7 @@ def test_argument_checks(oracle_mod):
         o.effective_C()
     assert e.value.status == oracle_mod.ERR_STATE
     with pytest.raises(oracle_mod.OracleError):
-        o.solve(6)
+        o.solve(7)
     with pytest.raises(oracle_mod.OracleError):
         o.solve(0, eps0=0.0)
     with pytest.raises(oracle_mod.OracleError):
