@@ -126,11 +126,11 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def make_image(workload, n_override=None):
+def make_image(workload, n_override=None, with_mask=False):
     w = WORKLOADS[workload]
     n = n_override or w["n"]
-    K, G, _ = getattr(inputs, w["gen"])(n=n)
-    return K, G, n
+    K, G, m = getattr(inputs, w["gen"])(n=n)
+    return (K, G, n, m) if with_mask else (K, G, n)
 
 
 def crop(K, G, m):
@@ -222,6 +222,9 @@ def main():
     ap.add_argument("--e2e-iters", type=int, default=50, help="PT iterations per load case in the host-buffer e2e call")
     ap.add_argument("--time-to-solution", action="store_true", help="also solve all six load cases to tol 1e-8")
     ap.add_argument("--tol", type=float, default=1e-8)
+    ap.add_argument("--st-factor", type=float, default=1.0, help="DR_ST_FACTOR (non-default tuning: 0.7 needs ~35 %% fewer iterations at 479^3)")
+    ap.add_argument("--void-rel", type=float, default=0.0, help="DR_VOID_REL (non-default: exact-void clamp of near-void cells)")
+    ap.add_argument("--tts-maxiter-n", type=int, default=100, help="time-to-solution: maxiter = this x n per load case")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -243,7 +246,8 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
 
-    K, G, n = make_image(args.workload, args.n)
+    K, G, n, mask = make_image(args.workload, args.n, with_mask=True)
+    mask = np.asarray(mask, dtype=bool) if mask is not None and np.shape(mask) == K.shape else None
     N = n ** 3
     Kd = torch.from_numpy(K).to(dev)
     Gd = torch.from_numpy(G).to(dev)
@@ -251,7 +255,12 @@ def main():
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
         # stag_tol 0: the timed dr_solve must run exactly K steps (the stagnation rule could end it early)
-        s = binding.Solver(Kd, Gd, stream=stream, ncheck=args.ncheck, kernel=args.kernel, form=args.form, palette=args.palette, stag_tol=0.0)
+        extra = {}
+        if args.st_factor != 1.0:
+            extra["st_factor"] = args.st_factor
+        if args.void_rel != 0.0:
+            extra["void_rel"] = args.void_rel
+        s = binding.Solver(Kd, Gd, stream=stream, ncheck=args.ncheck, kernel=args.kernel, form=args.form, palette=args.palette, stag_tol=0.0, **extra)
 
         def barrier():
             torch.cuda.synchronize(dev)
@@ -322,10 +331,29 @@ def main():
                    "h2d_bytes_per_step": 2 * N * 8 / nsteps, "d2h_bytes_per_step": (36 * 8 + 6 * 8 * (args.e2e_iters // args.ncheck)) / nsteps,
                    "call": "dr_solve_image_host (library defaults, DR_KERNEL 3): H2D K,G + dr_create + 6 load cases x %d iterations + C read back" % args.e2e_iters,
                    "seconds": dt}
+            # the same call for the image as a segmentation would deliver it: uint8 phase ids + per-phase tables
+            # (dr_solve_image_host_segmented: 1 byte per voxel over PCIe instead of 16)
+            if mask is not None:
+                ph = np.ascontiguousarray(mask, dtype=np.uint8)
+                Kt = np.array([K[~mask].flat[0] if (~mask).any() else 0.0, K[mask].flat[0] if mask.any() else 0.0])
+                Gt = np.array([G[~mask].flat[0] if (~mask).any() else 0.0, G[mask].flat[0] if mask.any() else 0.0])
+                if np.array_equal(Kt[ph], K) and np.array_equal(Gt[ph], G):
+                    Ph = torch.from_numpy(ph).pin_memory()
+                    stage8 = stage.view(torch.uint8)
+                    binding.solve_image_host_segmented(Ph, Kt, Gt, tol=1e-300, maxiter=3, ncheck=args.ncheck, stage=stage8, workspace=s.workspace)
+                    barrier()
+                    t0 = time.perf_counter()
+                    _, iters2, _ = binding.solve_image_host_segmented(Ph, Kt, Gt, eps0=args.eps0, tol=1e-300, maxiter=args.e2e_iters,
+                                                                      ncheck=args.ncheck, stage=stage8, workspace=s.workspace)
+                    torch.cuda.synchronize(dev)
+                    dt2 = shard.max_over_ranks((time.perf_counter() - t0) * 1e3, dist, dev) * 1e-3
+                    e2e["segmented"] = {"value": world * N * sum(iters2) / dt2, "unit": "voxel-updates/s", "seconds": dt2,
+                                        "h2d_bytes_per_step": N / sum(iters2), "call": "dr_solve_image_host_segmented (uint8 phase ids + tables)"}
+                    del Ph
             del stage, Kh, Gh
             # the solver's workspace was reused by the e2e call: rebuild the handle state
             s.close()
-            s = binding.Solver(Kd, Gd, stream=stream, workspace=s.workspace, ncheck=args.ncheck, kernel=args.kernel, form=args.form, palette=args.palette)
+            s = binding.Solver(Kd, Gd, stream=stream, workspace=s.workspace, ncheck=args.ncheck, kernel=args.kernel, form=args.form, palette=args.palette, **extra)
         if dist is not None:
             dist.barrier()
             dist.destroy_process_group()
@@ -337,9 +365,10 @@ def main():
         if args.time_to_solution and rank == 0:
             torch.cuda.synchronize(dev)
             t0 = time.perf_counter()
-            C, log = s.solve_all(args.eps0, args.tol, 100 * n)
+            C, log = s.solve_all(args.eps0, args.tol, args.tts_maxiter_n * n)
             torch.cuda.synchronize(dev)
             tts = {"seconds": time.perf_counter() - t0, "tol": args.tol, "driver": "six dr_solve calls on one handle",
+                   "params": dict(extra, form=args.form, kernel=args.kernel), "stop": [int(l[4]) for l in log] if len(log[0]) > 4 else None,
                    "iters": [l[1] for l in log], "status": [l[0] for l in log], "residual": [l[2] for l in log],
                    "C": [[float("%.6f" % v) for v in row] for row in C]}
             # the same six columns with all load cases in every launch (dr_solve_all) where six state
@@ -353,8 +382,8 @@ def main():
                 for rep in range(2):
                     torch.cuda.synchronize(dev)
                     t0 = time.perf_counter()
-                    b = binding.Solver(Kd, Gd, stream=stream, workspace=ws6, six=True, ncheck=args.ncheck, kernel=args.kernel, form=args.form, palette=args.palette)
-                    Cb, logb = b.solve_all_batched(args.eps0, args.tol, 100 * n)
+                    b = binding.Solver(Kd, Gd, stream=stream, workspace=ws6, six=True, ncheck=args.ncheck, kernel=args.kernel, form=args.form, palette=args.palette, **extra)
+                    Cb, logb = b.solve_all_batched(args.eps0, args.tol, args.tts_maxiter_n * n)
                     torch.cuda.synchronize(dev)
                     dtb = time.perf_counter() - t0
                     b.close()

@@ -107,6 +107,16 @@ dr_status dr_create(int nx, int ny, int nz, double h,
                     void* workspace, size_t workspace_bytes,
                     void* cuda_stream, dr_handle** out);
 
+/* The same for a SEGMENTED image, the usual product of CT segmentation (the marble image is a phase map):
+ * phase: DEVICE pointer, nx*ny*nz bytes, x fastest, phase id of every cell (0 .. nphase-1; an id >= nphase is DR_ERR_ARG);
+ * 1 <= nphase <= 256; K_table, G_table: HOST pointers, nphase doubles each (same value rules as dr_create).  The handle is
+ * identical, bit for bit, to the one dr_create builds from the expanded arrays K = K_table[phase], G = G_table[phase]; the
+ * caller moves 1 byte per cell instead of 16. */
+dr_status dr_create_segmented(int nx, int ny, int nz, double h,
+                              const unsigned char* phase, int nphase, const double* K_table, const double* G_table,
+                              void* workspace, size_t workspace_bytes,
+                              void* cuda_stream, dr_handle** out);
+
 /* Set a parameter (before dr_solve / dr_step).  Changing a parameter that shapes the iterate (DR_CFL, DR_ST_FACTOR,
  * DR_GAVG, DR_VOID_REL, DR_BC_MODE, DR_KERNEL, DR_FORM) discards the current fields: dr_iterate / dr_get_field return
  * DR_ERR_STATE until the next dr_step / dr_solve. */
@@ -184,6 +194,14 @@ dr_status dr_solve_image_host(int nx, int ny, int nz, double h,
                               double* stage_device, void* workspace, size_t workspace_bytes, void* cuda_stream,
                               double eps0, double tol, int maxiter, int ncheck,
                               double C_out[36], int iters_out[6]);
+
+/* dr_solve_image_host for a segmented image: phase_host (HOST, nx*ny*nz bytes) is staged through stage_device (DEVICE,
+ * >= nx*ny*nz bytes, caller-owned), then dr_create_segmented and the six load cases as above. */
+dr_status dr_solve_image_host_segmented(int nx, int ny, int nz, double h,
+                                        const unsigned char* phase_host, int nphase, const double* K_table, const double* G_table,
+                                        unsigned char* stage_device, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                                        double eps0, double tol, int maxiter, int ncheck,
+                                        double C_out[36], int iters_out[6]);
 
 /* Compliance (property) contribution tensor of the inclusions, Eq. 23: S* = S1 + phi H, i.e.
  * H = ((C*)^-1 - (C1)^-1) / phi.  Pure host post-processing of two effective tensors (the image and the matrix-only

@@ -17,7 +17,7 @@ CFL, ST_FACTOR, NCHECK, GAVG, VOID_REL, BC_MODE, KERNEL, ZCHUNK, FORM, PALETTE, 
 STOP_NONE, STOP_RESIDUAL, STOP_STAGNATION, STOP_MAXITER = range(4)
 PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_rel=VOID_REL, bc_mode=BC_MODE, kernel=KERNEL, zchunk=ZCHUNK, form=FORM, palette=PALETTE, stag_tol=STAG_TOL)
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
-EXPORTS = ("dr_workspace_bytes", "dr_workspace_bytes_six", "dr_solve_all", "dr_info_lc", "dr_create", "dr_set_param", "dr_solve", "dr_solve_six", "dr_effective_C_six", "dr_step", "dr_iterate",
+EXPORTS = ("dr_workspace_bytes", "dr_workspace_bytes_six", "dr_solve_all", "dr_info_lc", "dr_create", "dr_create_segmented", "dr_solve_image_host_segmented", "dr_set_param", "dr_solve", "dr_solve_six", "dr_effective_C_six", "dr_step", "dr_iterate",
            "dr_effective_C", "dr_avg_stress", "dr_offdiag_direct", "dr_info", "dr_get_field", "dr_solve_image_host", "dr_contribution_tensor",
            "dr_uses_palette", "dr_active_kernel", "dr_stop_reason", "dr_launch_count", "dr_last_error", "dr_destroy")
 
@@ -54,6 +54,10 @@ def lib():
             L.dr_offdiag_direct.argtypes = [vp, dp]
         L.dr_info.argtypes = [vp, C.POINTER(C.c_int), dp, dp]
         L.dr_get_field.argtypes = [vp, C.c_int, vp, C.c_size_t]
+        if hasattr(L, "dr_create_segmented"):
+            L.dr_create_segmented.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, vp, C.c_int, dp, dp, vp, C.c_size_t, vp, C.POINTER(vp)]
+            L.dr_solve_image_host_segmented.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, vp, C.c_int, dp, dp, vp, vp, C.c_size_t, vp,
+                                                        C.c_double, C.c_double, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
         L.dr_solve_image_host.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, vp, vp, vp, vp, C.c_size_t, vp,
                                           C.c_double, C.c_double, C.c_int, C.c_int, dp, C.POINTER(C.c_int)]
         if hasattr(L, "dr_contribution_tensor"):
@@ -93,13 +97,25 @@ def field_shape(nx, ny, nz, f):
 class Solver:
     """dr_create .. dr_destroy.  K, G: torch.float64 CUDA tensors of shape (nz, ny, nx), x fastest."""
 
-    def __init__(self, K, G, h=1.0, stream=None, workspace=None, six=False, **params):
+    def __init__(self, K, G, h=1.0, stream=None, workspace=None, six=False, phase=None, **params):
+        """K, G: the modulus fields -- or, with phase= (torch.uint8 CUDA tensor (nz, ny, nx) of phase ids), the per-phase
+        tables (sequences of nphase floats): dr_create_segmented."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libdr needs a CUDA device (there is no CPU fallback)")
-        if not (K.is_cuda and G.is_cuda and K.dtype == torch.float64 and G.dtype == torch.float64):
+        if phase is not None:
+            if not (phase.is_cuda and phase.dtype == torch.uint8 and phase.dim() == 3):
+                raise TypeError("phase must be a uint8 CUDA tensor of shape (nz, ny, nx)")
+            import numpy as np
+            Kt = np.ascontiguousarray(K, dtype=np.float64).ravel()
+            Gt = np.ascontiguousarray(G, dtype=np.float64).ravel()
+            assert Kt.size == Gt.size
+            K = phase
+        elif not (K.is_cuda and G.is_cuda and K.dtype == torch.float64 and G.dtype == torch.float64):
             raise TypeError("K and G must be float64 CUDA tensors")
-        assert K.dim() == 3 and K.shape == G.shape
+        else:
+            assert K.shape == G.shape
+        assert K.dim() == 3
         self.nz, self.ny, self.nx = (int(s) for s in K.shape)
         self.device = K.device
         self._torch = torch
@@ -116,10 +132,17 @@ class Solver:
         self.stream.wait_stream(torch.cuda.current_stream(K.device))
         with torch.cuda.device(K.device), torch.cuda.stream(self.stream):
             K = K.contiguous()
-            G = G.contiguous()
-            st = lib().dr_create(self.nx, self.ny, self.nz, float(h), K.data_ptr(), G.data_ptr(),
-                                 workspace.data_ptr(), workspace.numel() * workspace.element_size(),
-                                 self.stream.cuda_stream, C.byref(self._h))
+            if phase is not None:
+                dp = C.POINTER(C.c_double)
+                st = lib().dr_create_segmented(self.nx, self.ny, self.nz, float(h), K.data_ptr(), int(Kt.size),
+                                               Kt.ctypes.data_as(dp), Gt.ctypes.data_as(dp),
+                                               workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                               self.stream.cuda_stream, C.byref(self._h))
+            else:
+                G = G.contiguous()
+                st = lib().dr_create(self.nx, self.ny, self.nz, float(h), K.data_ptr(), G.data_ptr(),
+                                     workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                     self.stream.cuda_stream, C.byref(self._h))
         if st != OK:
             raise DrError(st, "dr_create failed (status %d)" % st)
         for k, v in params.items():
@@ -201,7 +224,7 @@ class Solver:
         for lc in range(6):
             st = self.solve(lc, eps0, tol, maxiter)
             it, r, ms = self.info()
-            log.append((st, it, r, ms))
+            log.append((st, it, r, ms, self.stop_reason()))
         return self.effective_C(), log
 
     def close(self):
@@ -278,3 +301,33 @@ def solve_image_host(K_host, G_host, h=1.0, eps0=1e-4, tol=1e-8, maxiter=100000,
     if st not in (OK, MAXITER):
         raise DrError(st, "dr_solve_image_host failed")
     return Cout.reshape(6, 6), list(iters), st
+
+
+def solve_image_host_segmented(phase_host, K_table, G_table, h=1.0, eps0=1e-4, tol=1e-8, maxiter=100000, ncheck=0,
+                               stage=None, workspace=None, device="cuda:0", six=False):
+    """dr_solve_image_host_segmented: HOST uint8 phase ids (numpy or CPU torch tensor, (nz,ny,nx)) + per-phase tables.
+    Returns (C, iters, status)."""
+    import numpy as np
+    import torch
+    Pt = torch.as_tensor(phase_host)
+    assert Pt.dtype == torch.uint8 and Pt.is_contiguous() and not Pt.is_cuda and Pt.dim() == 3
+    nz, ny, nx = (int(s) for s in Pt.shape)
+    N = nx * ny * nz
+    Kt = np.ascontiguousarray(K_table, dtype=np.float64).ravel()
+    Gt = np.ascontiguousarray(G_table, dtype=np.float64).ravel()
+    assert Kt.size == Gt.size
+    if stage is None:
+        stage = torch.empty(N, dtype=torch.uint8, device=device)
+    if workspace is None:
+        workspace = torch.empty(workspace_bytes(nx, ny, nz, six), dtype=torch.uint8, device=device)
+    Cout = np.zeros(36)
+    iters = (C.c_int * 6)()
+    dp = C.POINTER(C.c_double)
+    with torch.cuda.device(stage.device):
+        st = lib().dr_solve_image_host_segmented(nx, ny, nz, float(h), Pt.data_ptr(), int(Kt.size), Kt.ctypes.data_as(dp), Gt.ctypes.data_as(dp),
+                                                 stage.data_ptr(), workspace.data_ptr(), workspace.numel(), torch.cuda.current_stream().cuda_stream,
+                                                 eps0, tol, maxiter, ncheck, Cout.ctypes.data_as(dp), iters)
+    if st not in (OK, MAXITER):
+        raise DrError(st, "dr_solve_image_host_segmented failed (status %d)" % st)
+    return Cout.reshape(6, 6), list(iters), st
+

@@ -256,11 +256,14 @@ static cudaError_t set_kernel_attributes(int device) {
     return e;
 }
 
-extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K, const double* G,
-                               void* workspace, size_t workspace_bytes, void* cuda_stream, dr_handle** out) {
+// dr_create and dr_create_segmented: the moduli come from dense fp64 arrays (K, G) or from phase ids + host tables
+static dr_status create_impl(int nx, int ny, int nz, double h, const double* K, const double* G,
+                             const unsigned char* phase, int nphase, const double* K_table, const double* G_table,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream, dr_handle** out) {
     if (!out) return DR_ERR_ARG;
     *out = nullptr;
-    if (!sizes_ok(nx, ny, nz) || !(h > 0.0) || !std::isfinite(h) || !K || !G) return DR_ERR_ARG;
+    if (!sizes_ok(nx, ny, nz) || !(h > 0.0) || !std::isfinite(h)) return DR_ERR_ARG;
+    if (phase ? (nphase < 1 || nphase > 256 || !K_table || !G_table) : (!K || !G)) return DR_ERR_ARG;
     if (!workspace || ((uintptr_t)workspace & 255u) || workspace_bytes < dr_workspace_bytes(nx, ny, nz)) return DR_ERR_WORKSPACE;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return DR_ERR_CUDA; }
@@ -317,8 +320,18 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
         // state fields and moduli boxes start as zeros (halo nodes are never written afterwards)
         if (!cuda_ok(H, cudaMemsetAsync(workspace, 0, H->nsets == 6 ? dr_workspace_bytes_six(nx, ny, nz) : dr_workspace_bytes(nx, ny, nz), H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }
         if (!cuda_ok(H, cudaMemsetAsync(H->palK, 0xff, 4096, H->st), "cudaMemsetAsync")) { st = DR_ERR_CUDA; break; }     // palK and palG := EMPTY
+        DrModSrc src;
+        src.K = K; src.G = G; src.ids = phase; src.tab = nullptr; src.nphase = nphase;
+        if (phase) {
+            // the caller's tables go to the (not yet used) table block of the coded path: K at 0, G at 256
+            double host_tab[512];
+            for (int e = 0; e < 256; ++e) { host_tab[e] = e < nphase ? K_table[e] : 0.0; host_tab[256 + e] = e < nphase ? G_table[e] : 0.0; }
+            if (!cuda_ok(H, cudaMemcpyAsync(H->tabs, host_tab, sizeof(host_tab), cudaMemcpyHostToDevice, H->st), "cudaMemcpyAsync(tables)") ||
+                !cuda_ok(H, cudaStreamSynchronize(H->st), "cudaStreamSynchronize")) { st = DR_ERR_CUDA; break; }      // host_tab is a stack buffer
+            src.tab = H->tabs;
+        }
         dim3 blk(64, 4, 1), grd((nx + 2 + 63) / 64, (ny + 2 + 3) / 4, nz + 2);
-        k_pad_moduli<<<grd, blk, 0, H->st>>>(H->L, K, G, H->K0, H->G0, H->flags, H->hmax_bits);
+        k_pad_moduli<<<grd, blk, 0, H->st>>>(H->L, src, H->K0, H->G0, H->flags, H->hmax_bits);
         H->launches++;
         if (!cuda_ok(H, cudaGetLastError(), "k_pad_moduli")) { st = DR_ERR_CUDA; break; }
         const long long cnt = H->L.count;
@@ -328,7 +341,7 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
         // palette of the distinct (K,G) pairs; more than 256 of them (flag 2) simply leaves the fp64 path in charge
         {
             const long long Ncell = (long long)nx * ny * nz;
-            k_pal_build<<<(unsigned)((Ncell + 255) / 256), 256, 0, H->st>>>(Ncell, K, G, H->palK, H->palG, H->flags);
+            k_pal_build<<<(unsigned)((Ncell + 255) / 256), 256, 0, H->st>>>(Ncell, src, H->palK, H->palG, H->flags);
             H->launches++;
             if (!cuda_ok(H, cudaGetLastError(), "k_pal_build")) { st = DR_ERR_CUDA; break; }
         }
@@ -338,7 +351,7 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
             !cuda_ok(H, cudaStreamSynchronize(H->st), "cudaStreamSynchronize")) { st = DR_ERR_CUDA; break; }
         if (fl & 1u) { st = DR_ERR_ARG; break; }
         if (!(fl & 2u)) {
-            k_pal_assign<<<dim3(tiles_x(H->L), tiles_y(H->L), nz + 3), dim3(FUSED_TX, FUSED_TY, 1), 0, H->st>>>(H->L, K, G, H->palK, H->palG, H->ids, H->flags);
+            k_pal_assign<<<dim3(tiles_x(H->L), tiles_y(H->L), nz + 3), dim3(FUSED_TX, FUSED_TY, 1), 0, H->st>>>(H->L, src, H->palK, H->palG, H->ids, H->flags);
             k_pal_values<<<1, 256, 0, H->st>>>(H->palK, H->palG, H->pal, 0.0);
             H->launches += 2;
             unsigned int fl2 = 0;
@@ -360,6 +373,18 @@ extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K
     }
     *out = H;
     return DR_OK;
+}
+
+extern "C" dr_status dr_create(int nx, int ny, int nz, double h, const double* K, const double* G,
+                               void* workspace, size_t workspace_bytes, void* cuda_stream, dr_handle** out) {
+    return create_impl(nx, ny, nz, h, K, G, nullptr, 0, nullptr, nullptr, workspace, workspace_bytes, cuda_stream, out);
+}
+
+extern "C" dr_status dr_create_segmented(int nx, int ny, int nz, double h, const unsigned char* phase, int nphase,
+                                         const double* K_table, const double* G_table,
+                                         void* workspace, size_t workspace_bytes, void* cuda_stream, dr_handle** out) {
+    if (!phase) return DR_ERR_ARG;
+    return create_impl(nx, ny, nz, h, nullptr, nullptr, phase, nphase, K_table, G_table, workspace, workspace_bytes, cuda_stream, out);
 }
 
 extern "C" dr_status dr_set_param(dr_handle* H, int id, double v) {
@@ -1007,18 +1032,9 @@ extern "C" dr_status dr_get_field(dr_handle* H, int field, double* dst, size_t n
     return DR_OK;
 }
 
-extern "C" dr_status dr_solve_image_host(int nx, int ny, int nz, double h, const double* K_host, const double* G_host,
-                                         double* stage_device, void* workspace, size_t workspace_bytes, void* cuda_stream,
-                                         double eps0, double tol, int maxiter, int ncheck, double C_out[36], int iters_out[6]) {
-    if (!sizes_ok(nx, ny, nz) || !K_host || !G_host || !stage_device || !C_out) return DR_ERR_ARG;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t N = (size_t)nx * ny * nz;
-    if (cudaMemcpyAsync(stage_device, K_host, N * sizeof(double), cudaMemcpyHostToDevice, st) != cudaSuccess) return DR_ERR_CUDA;
-    if (cudaMemcpyAsync(stage_device + N, G_host, N * sizeof(double), cudaMemcpyHostToDevice, st) != cudaSuccess) return DR_ERR_CUDA;
-    dr_handle* H = nullptr;
-    dr_status s = dr_create(nx, ny, nz, h, stage_device, stage_device + N, workspace, workspace_bytes, cuda_stream, &H);
-    if (s != DR_OK) return s;
-    dr_status worst = DR_OK;
+// the six load cases of a freshly created handle -> C_out; destroys the handle
+static dr_status solve_image(dr_handle* H, double eps0, double tol, int maxiter, int ncheck, double C_out[36], int iters_out[6]) {
+    dr_status s, worst = DR_OK;
     if (ncheck > 0) dr_set_param(H, DR_NCHECK, ncheck);
     if (H->nsets == 6) {                             // workspace of dr_workspace_bytes_six: all six load cases per launch
         s = dr_solve_all(H, eps0, tol, maxiter, nullptr);
@@ -1035,6 +1051,34 @@ extern "C" dr_status dr_solve_image_host(int nx, int ny, int nz, double h, const
     s = dr_effective_C(H, C_out);
     dr_destroy(H);
     return s != DR_OK ? s : worst;
+}
+
+extern "C" dr_status dr_solve_image_host(int nx, int ny, int nz, double h, const double* K_host, const double* G_host,
+                                         double* stage_device, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                                         double eps0, double tol, int maxiter, int ncheck, double C_out[36], int iters_out[6]) {
+    if (!sizes_ok(nx, ny, nz) || !K_host || !G_host || !stage_device || !C_out) return DR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t N = (size_t)nx * ny * nz;
+    if (cudaMemcpyAsync(stage_device, K_host, N * sizeof(double), cudaMemcpyHostToDevice, st) != cudaSuccess) return DR_ERR_CUDA;
+    if (cudaMemcpyAsync(stage_device + N, G_host, N * sizeof(double), cudaMemcpyHostToDevice, st) != cudaSuccess) return DR_ERR_CUDA;
+    dr_handle* H = nullptr;
+    dr_status s = dr_create(nx, ny, nz, h, stage_device, stage_device + N, workspace, workspace_bytes, cuda_stream, &H);
+    if (s != DR_OK) return s;
+    return solve_image(H, eps0, tol, maxiter, ncheck, C_out, iters_out);
+}
+
+extern "C" dr_status dr_solve_image_host_segmented(int nx, int ny, int nz, double h, const unsigned char* phase_host, int nphase,
+                                                   const double* K_table, const double* G_table,
+                                                   unsigned char* stage_device, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                                                   double eps0, double tol, int maxiter, int ncheck, double C_out[36], int iters_out[6]) {
+    if (!sizes_ok(nx, ny, nz) || !phase_host || !stage_device || !C_out) return DR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t N = (size_t)nx * ny * nz;
+    if (cudaMemcpyAsync(stage_device, phase_host, N, cudaMemcpyHostToDevice, st) != cudaSuccess) return DR_ERR_CUDA;
+    dr_handle* H = nullptr;
+    dr_status s = dr_create_segmented(nx, ny, nz, h, stage_device, nphase, K_table, G_table, workspace, workspace_bytes, cuda_stream, &H);
+    if (s != DR_OK) return s;
+    return solve_image(H, eps0, tol, maxiter, ncheck, C_out, iters_out);
 }
 
 // 6x6 inverse by Gauss-Jordan elimination with partial pivoting (host); false if singular

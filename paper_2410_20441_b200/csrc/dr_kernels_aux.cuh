@@ -17,9 +17,26 @@ __device__ __forceinline__ double dr_u0(const DrPT& P, int a, double x, double y
 }
 
 // ------------------------------------------------------------------------------------------------------
-// a0: copy the caller's dense K,G into the padded box with a replicate halo; validate; max of K+4G/3.
+// where the moduli of cell s come from: dense fp64 arrays (dr_create), or a segmented image = one uint8 phase id per
+// cell + a table tab[0..255] = K, tab[256..511] = G (dr_create_segmented).  bad: id outside the table.
+struct DrModSrc { const double* K; const double* G; const unsigned char* ids; const double* tab; int nphase; };
+
+__device__ __forceinline__ void dr_src_get(const DrModSrc& S, size_t s, double& Kv, double& Gv, bool& bad) {
+    // + 0.0 turns a -0.0 modulus into +0.0 (it passes the >= 0 test): 1/(-0) = -inf next to a +0 cell would make
+    // the edge mean inf - inf = NaN, and its bit pattern would win the unsigned max of hmax
+    if (S.ids) {
+        int id = S.ids[s];
+        if (id >= S.nphase) { bad = true; id = 0; }
+        Kv = S.tab[id] + 0.0; Gv = S.tab[256 + id] + 0.0;
+    } else {
+        Kv = S.K[s] + 0.0; Gv = S.G[s] + 0.0;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// a0: copy the caller's moduli into the padded box with a replicate halo; validate; max of K+4G/3.
 // flags[0] |= 1 if any modulus is negative or not finite.  hmax_bits: atomicMax on the bit pattern.
-__global__ void k_pad_moduli(DrLayout L, const double* __restrict__ Ksrc, const double* __restrict__ Gsrc,
+__global__ void k_pad_moduli(DrLayout L, DrModSrc S,
                              double* __restrict__ Kp, double* __restrict__ Gp,
                              unsigned int* flags, unsigned long long* hmax_bits) {
     int i = blockIdx.x * blockDim.x + threadIdx.x - 1;      // -1 .. nx
@@ -28,13 +45,13 @@ __global__ void k_pad_moduli(DrLayout L, const double* __restrict__ Ksrc, const 
     if (i > L.nx || j > L.ny) return;
     int ci = min(max(i, 0), L.nx - 1), cj = min(max(j, 0), L.ny - 1), ck = min(max(k, 0), L.nz - 1);
     size_t s = (size_t)ci + (size_t)L.nx * ((size_t)cj + (size_t)L.ny * ck);
-    // + 0.0 turns a -0.0 modulus into +0.0 (it passes the >= 0 test below): 1/(-0) = -inf next to a +0 cell would make
-    // the edge mean inf - inf = NaN, and its bit pattern would win the unsigned max of hmax
-    double Kv = Ksrc[s] + 0.0, Gv = Gsrc[s] + 0.0;
+    double Kv, Gv;
+    bool bad = false;
+    dr_src_get(S, s, Kv, Gv, bad);
     long long q = L.origin + i + L.sy * j + L.sz * k;
     Kp[q] = Kv; Gp[q] = Gv;
     if (i == ci && j == cj && k == ck) {
-        bool bad = !(Kv >= 0.0) || !(Gv >= 0.0) || isinf(Kv) || isinf(Gv);
+        bad = bad || !(Kv >= 0.0) || !(Gv >= 0.0) || isinf(Kv) || isinf(Gv);
         if (bad) atomicOr(flags, 1u);
         else {
             double Hc = Kv + 4.0 * Gv / 3.0;
@@ -261,14 +278,16 @@ __device__ __forceinline__ int dr_pal_find(const unsigned long long* kK, const u
 }
 
 // pass 1: every cell inserts its pair (consecutive equal cells are skipped); flags[0] |= 2 when the table overflows
-__global__ void k_pal_build(long long N, const double* __restrict__ Ksrc, const double* __restrict__ Gsrc,
-                            unsigned long long* kK, unsigned long long* kG, unsigned int* flags) {
+__global__ void k_pal_build(long long N, DrModSrc S, unsigned long long* kK, unsigned long long* kG, unsigned int* flags) {
     const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= N || (*((volatile unsigned int*)flags) & 2u)) return;
-    // + 0.0: -0.0 and +0.0 are the same modulus (see k_pad_moduli)
-    const unsigned long long kb = (unsigned long long)__double_as_longlong(Ksrc[q] + 0.0), gb = (unsigned long long)__double_as_longlong(Gsrc[q] + 0.0);
+    double Kv, Gv, Kl, Gl;
+    bool bad = false;
+    dr_src_get(S, (size_t)q, Kv, Gv, bad);
+    const unsigned long long kb = (unsigned long long)__double_as_longlong(Kv), gb = (unsigned long long)__double_as_longlong(Gv);
     if (q > 0 && (threadIdx.x & 31) != 0) {          // same pair as the previous cell of the warp: that lane inserts it
-        if ((unsigned long long)__double_as_longlong(Ksrc[q - 1] + 0.0) == kb && (unsigned long long)__double_as_longlong(Gsrc[q - 1] + 0.0) == gb) return;
+        dr_src_get(S, (size_t)(q - 1), Kl, Gl, bad);
+        if ((unsigned long long)__double_as_longlong(Kl) == kb && (unsigned long long)__double_as_longlong(Gl) == gb) return;
     }
     if (dr_pal_insert(kK, kG, kb, gb) < 0) atomicOr(flags, 2u);
 }
@@ -276,7 +295,7 @@ __global__ void k_pal_build(long long N, const double* __restrict__ Ksrc, const 
 // pass 2: phase ids, TILE-BLOCKED for the fused kernel: block (bx, by, z) holds the TX*TY ids of the extended tile
 // (i0-1+tx, j0-1+ty) of layer z-1, i0 = bx (TX-2), j0 = by (TY-2), replicate-padded like the moduli; flags[0] |= 4 on a miss.
 // grid (gx, gy, nz+3), block (TX, TY).
-__global__ void k_pal_assign(DrLayout L, const double* __restrict__ Ksrc, const double* __restrict__ Gsrc,
+__global__ void k_pal_assign(DrLayout L, DrModSrc S,
                              const unsigned long long* __restrict__ kK, const unsigned long long* __restrict__ kG,
                              unsigned char* __restrict__ ids, unsigned int* flags) {
     const int TX = blockDim.x, TY = blockDim.y;
@@ -285,7 +304,10 @@ __global__ void k_pal_assign(DrLayout L, const double* __restrict__ Ksrc, const 
     const int k = (int)blockIdx.z - 1;
     const int ci = min(max(i, 0), L.nx - 1), cj = min(max(j, 0), L.ny - 1), ck = min(max(k, 0), L.nz - 1);
     const size_t s = (size_t)ci + (size_t)L.nx * ((size_t)cj + (size_t)L.ny * ck);
-    const int slot = dr_pal_find(kK, kG, (unsigned long long)__double_as_longlong(Ksrc[s] + 0.0), (unsigned long long)__double_as_longlong(Gsrc[s] + 0.0));
+    double Kv, Gv;
+    bool bad = false;
+    dr_src_get(S, s, Kv, Gv, bad);
+    const int slot = dr_pal_find(kK, kG, (unsigned long long)__double_as_longlong(Kv), (unsigned long long)__double_as_longlong(Gv));
     if (slot < 0) { atomicOr(flags, 4u); return; }
     const size_t blk = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
     ids[blk * (size_t)(TX * TY) + threadIdx.y * TX + threadIdx.x] = (unsigned char)slot;

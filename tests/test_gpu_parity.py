@@ -466,3 +466,40 @@ def test_triaxial_load_case_and_eq27_29_vs_oracle(oracle_mod, gpu):
     C = s.effective_C()
     sym = np.array([0.5 * (C[0, 1] + C[1, 0]), 0.5 * (C[0, 2] + C[2, 0]), 0.5 * (C[1, 2] + C[2, 1])])
     assert np.max(np.abs(d - sym)) <= 1e-6 * C[0, 0]
+
+
+# ------------------------------------------------------------------------------------------------ segmented images (phase ids + tables)
+def test_segmented_create_is_bitwise_the_fp64_create(oracle_mod, gpu):
+    """dr_create_segmented (uint8 phase ids + per-phase tables) builds the same handle as dr_create on the expanded arrays:
+    identical fields after a fixed iteration count (hence the oracle parity of the fp64 path carries over), identical C from
+    the host-buffer call; ids outside the table and bad table sizes are refused."""
+    import torch
+    rng = np.random.default_rng(11)
+    shape = (23, 31, 40)                                  # (nz, ny, nx)
+    Kt = np.array([37.0, 5.0, 0.0, 2.2, 70.2]); Gt = np.array([44.0, 2.0, 0.0, 0.0, 29.0])     # matrix, soft, void, fluid, calcite
+    ph = rng.integers(0, 5, size=shape).astype(np.uint8)
+    K, G = np.ascontiguousarray(Kt[ph]), np.ascontiguousarray(Gt[ph])
+    a = gpu.Solver(to_dev(K), to_dev(G))
+    b = gpu.Solver(Kt, Gt, phase=torch.from_numpy(ph).cuda())
+    for lc, n in ((1, 7), (5, 10)):
+        a.step(lc, 1e-4, n); b.step(lc, 1e-4, n)
+        assert a.active_kernel() == b.active_kernel() == 3 and b.uses_palette()
+        for f in range(9):
+            assert torch.equal(a.get_field(f), b.get_field(f)), (lc, f)
+        assert a.info()[1] == b.info()[1] and np.array_equal(a.avg_stress(), b.avg_stress())
+    o = oracle_mod.Oracle(K, G)
+    o.step(5, 1e-4, 10)
+    assert max(field_errors(o, b, K, G, 1e-4)) <= FIELD_TOL
+    Ca, ia, sa = gpu.solve_image_host(K, G, tol=1e-7, maxiter=3000, ncheck=50)
+    Cb, ib, sb = gpu.solve_image_host_segmented(ph, Kt, Gt, tol=1e-7, maxiter=3000, ncheck=50)
+    Cc, ic, sc = gpu.solve_image_host_segmented(ph, Kt, Gt, tol=1e-7, maxiter=3000, ncheck=50, six=True)
+    assert sa == sb == sc == 0 and ia == ib == ic and np.array_equal(Ca, Cb) and np.array_equal(Ca, Cc)
+    with pytest.raises(gpu.DrError) as e:                 # an id beyond the table
+        gpu.Solver(Kt[:4], Gt[:4], phase=torch.from_numpy(ph).cuda())
+    assert e.value.status == gpu.ERR_ARG
+    with pytest.raises(gpu.DrError) as e:                 # more than 256 phases
+        gpu.Solver(np.ones(257), np.ones(257), phase=torch.from_numpy(ph).cuda())
+    assert e.value.status == gpu.ERR_ARG
+    with pytest.raises(gpu.DrError) as e:                 # negative modulus in the table
+        gpu.Solver(np.array([1.0, -1.0, 1.0, 1.0, 1.0]), Gt, phase=torch.from_numpy(ph).cuda())
+    assert e.value.status == gpu.ERR_ARG
