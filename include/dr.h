@@ -17,6 +17,7 @@
  *  - Load cases 0..5 apply the displacement gradient D with one non-zero entry eps0:
  *      0: Dxx  1: Dyy  2: Dzz  (normal compression tests, App. A.1)
  *      3: u_y = eps0 z   4: u_x = eps0 z   5: u_x = eps0 y   (simple shear tests, App. A.2)
+ *    Load case 6 (dr_solve / dr_step only) is the 7th, triaxial test of App. A.3: Dxx = Dyy = Dzz = eps0 (dr_offdiag_direct).
  *  - Units of C* are the units of K and G.
  *  - The library allocates NO device memory: the caller passes one workspace of dr_workspace_bytes() bytes
  *    (e.g. a torch tensor) that is borrowed until dr_destroy.  K and G are borrowed during dr_create only.
@@ -62,8 +63,9 @@ typedef enum {
                           (baseline); 2 fused z-march kernel with register-prefetched LDG loads;
                           3 [default] temporal blocking: TWO PT iterations per sweep (the state is read and written once per two
                           iterations) on stencil-coded images -- images with <= 256 distinct (K,G) pairs, edge moduli
-                          and node stiffnesses, i.e. segmented rock images; other images, odd leftovers and a check
-                          iteration that is the first of a pair run kernel 0 (dr_active_kernel tells), and so does DR_FORM 1;
+                          and node stiffnesses, i.e. segmented rock images; odd leftovers and a check iteration that
+                          would be the first of a pair run one iteration of the same coded kernel; images that cannot be
+                          coded run kernel 0 (dr_active_kernel tells), and so does DR_FORM 1;
                           4 one iteration per sweep with the coded kernel (A/B reference of 3)                          */
     DR_ZCHUNK = 7,     /* z layers per CTA of the fused kernels; 0 = automatic [default] (tuning knob)            */
     DR_PALETTE = 9,    /* 1 [default]: images with <= 256 distinct (K,G) pairs run the fused kernel on a uint8 phase id

@@ -53,10 +53,12 @@ def zslab_bounds(nz: int, world: int, rank: int):
     return k0, k0 + q + (1 if rank < r else 0)
 
 
-def zslab_extent(nz: int, world: int, rank: int):
-    """cell layers [e0, e1) the rank holds: its own plus one ghost layer towards every neighbour"""
+def zslab_extent(nz: int, world: int, rank: int, depth: int = 1):
+    """cell layers [e0, e1) the rank holds: its own plus `depth` ghost layers towards every neighbour"""
     k0, k1 = zslab_bounds(nz, world, rank)
-    return (k0 - 1 if rank > 0 else k0), (k1 + 1 if rank < world - 1 else k1)
+    if depth < 1 or nz < (depth + 1) * world:
+        raise ValueError("need depth >= 1 and more owned layers per rank than ghost layers")
+    return (k0 - depth if rank > 0 else k0), (k1 + depth if rank < world - 1 else k1)
 
 
 def zslab_halo_plan(nz: int, world: int, rank: int):
@@ -95,3 +97,31 @@ def zslab_exchange(get_plane, set_plane, plan, dist):
     for recv, inn in landing:
         for (f, z), t in zip(recv, inn):
             set_plane(f, z, t)
+
+
+# Deeper ghost zones: one exchange per `depth` PT iterations (depth 2 is what the two-iterations-per-sweep kernel needs).
+# After `depth` iterations without exchange the error of the artificial wall has travelled through the whole ghost zone but
+# not into the owned range (one iteration moves it by at most one layer: the stress update reads velocities of the same and
+# the next layer, the velocity update reads stresses of the same and the previous face).  The plan is therefore the plain
+# refresh of the ghost zone: every field of the `depth` ghost cell layers and of the `depth` faces beyond the interface face.
+
+def zslab_refresh_plan(nz: int, world: int, rank: int, depth: int, layer_fields, face_fields):
+    """For every neighbour: (peer, send, recv) as in zslab_halo_plan, for an exchange every `depth` iterations.
+    layer_fields / face_fields: names of the state arrays that live on cell layers / on z faces."""
+    k0, k1 = zslab_bounds(nz, world, rank)
+    e0, _ = zslab_extent(nz, world, rank, depth)
+    plan = []
+    if rank > 0:
+        # I own layers k0 .. and faces k0 ..; the lower neighbour's ghost zone is my layers k0 .. k0+depth-1 and my faces
+        # k0+1 .. k0+depth; mine is its layers k0-depth .. k0-1 and faces k0-depth .. k0-1
+        send = [(f, k0 + d - e0) for d in range(depth) for f in layer_fields] + [(f, k0 + 1 + d - e0) for d in range(depth) for f in face_fields]
+        recv = [(f, k0 - depth + d - e0) for d in range(depth) for f in layer_fields] + [(f, k0 - depth + d - e0) for d in range(depth) for f in face_fields]
+        plan.append((rank - 1, send, recv))
+    if rank < world - 1:
+        # the upper neighbour's ghost zone is my layers k1-depth .. k1-1 and my faces k1-depth .. k1-1; mine is its layers
+        # k1 .. k1+depth-1 and faces k1+1 .. k1+depth
+        send = [(f, k1 - depth + d - e0) for d in range(depth) for f in layer_fields] + [(f, k1 - depth + d - e0) for d in range(depth) for f in face_fields]
+        recv = [(f, k1 + d - e0) for d in range(depth) for f in layer_fields] + [(f, k1 + 1 + d - e0) for d in range(depth) for f in face_fields]
+        plan.append((rank + 1, send, recv))
+    return plan
+

@@ -64,7 +64,7 @@ def test_zslab_partition_covers_every_layer_once():
         shard.zslab_bounds(3, 2, 0)
 
 
-def _slab_worker(rank, world, port, out, nz, niter, lc):
+def _slab_worker(rank, world, port, out, nz, niter, lc, depth=1):
     import numpy as np
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
@@ -78,7 +78,7 @@ def _slab_worker(rank, world, port, out, nz, niter, lc):
     ref = dro.Oracle(K, G)
     ref.step(lc, 1e-4, 0)
     k0, k1 = shard.zslab_bounds(nz, world, rank)
-    e0, e1 = shard.zslab_extent(nz, world, rank)
+    e0, e1 = shard.zslab_extent(nz, world, rank, depth)
     mine = dro.Oracle(K[e0:e1], G[e0:e1])
     mine.step(lc, 1e-4, 0)                              # allocates the slab state (its own affine start is overwritten next)
 
@@ -89,7 +89,10 @@ def _slab_worker(rank, world, port, out, nz, niter, lc):
     for name in dro.Oracle.RAW:
         a = ref.get_raw(name)
         mine.set_raw(name, a[e0:e1 + 1] if face_fields(name) else a[e0:e1])
-    plan = shard.zslab_halo_plan(nz, world, rank)
+    layer_f = [n for n in dro.Oracle.RAW if not face_fields(n)]
+    face_f = [n for n in dro.Oracle.RAW if face_fields(n)]
+    plan = shard.zslab_halo_plan(nz, world, rank) if depth == 1 else shard.zslab_refresh_plan(nz, world, rank, depth, layer_f, face_f)
+    moved = [f for f, _ in shard.ZSLAB_HALO_FIELDS] if depth == 1 else list(dro.Oracle.RAW)
     cache = {}
 
     def get_plane(f, z):
@@ -98,11 +101,12 @@ def _slab_worker(rank, world, port, out, nz, niter, lc):
     def set_plane(f, z, t):
         cache[f][z] = t.numpy()
 
-    for it in range(niter):
-        mine.iterate(lc, 1e-4, 1)
-        cache = {f: mine.get_raw(f) for f, _ in shard.ZSLAB_HALO_FIELDS}
+    assert niter % depth == 0
+    for it in range(niter // depth):
+        mine.iterate(lc, 1e-4, depth)                   # `depth` iterations per exchange
+        cache = {f: mine.get_raw(f) for f in moved}
         shard.zslab_exchange(get_plane, set_plane, plan, dist)
-        for f, _ in shard.ZSLAB_HALO_FIELDS:
+        for f in moved:
             mine.set_raw(f, cache[f])
     ref.iterate(lc, 1e-4, niter)
     ok = True
@@ -140,3 +144,22 @@ def test_two_rank_zslab_halo_exchange_reproduces_the_single_domain_iterate(oracl
         assert p.exitcode == 0
     assert all(g[1] for g in got), got
     assert all(g[2] for g in got), got
+
+
+@pytest.mark.parametrize("depth,world,nz", [(2, 2, 17), (2, 3, 19), (3, 2, 16)])
+def test_zslab_deeper_ghost_zone_one_exchange_per_sweep_of_several_iterations(oracle_mod, depth, world, nz):
+    """what the two-iterations-per-sweep kernel needs (depth 2): `depth` ghost layers per interface, `depth` PT iterations
+    between exchanges, the whole ghost zone refreshed (shard.zslab_refresh_plan).  Every owned value equals the
+    single-domain oracle's bit for bit after 12 iterations; three ranks exercise a slab with two neighbours."""
+    port = _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    ps = [ctx.Process(target=_slab_worker, args=(r, world, port, q, nz, 12, 2, depth)) for r in range(world)]
+    for p in ps:
+        p.start()
+    got = sorted(q.get(timeout=300) for _ in range(world))
+    for p in ps:
+        p.join(120)
+        assert p.exitcode == 0
+    assert all(g[1] for g in got) and all(g[2] for g in got), got
+
