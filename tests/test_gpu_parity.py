@@ -490,10 +490,11 @@ def test_segmented_create_is_bitwise_the_fp64_create(oracle_mod, gpu):
     o = oracle_mod.Oracle(K, G)
     o.step(5, 1e-4, 10)
     assert max(field_errors(o, b, K, G, 1e-4)) <= FIELD_TOL
-    Ca, ia, sa = gpu.solve_image_host(K, G, tol=1e-7, maxiter=3000, ncheck=50)
-    Cb, ib, sb = gpu.solve_image_host_segmented(ph, Kt, Gt, tol=1e-7, maxiter=3000, ncheck=50)
-    Cc, ic, sc = gpu.solve_image_host_segmented(ph, Kt, Gt, tol=1e-7, maxiter=3000, ncheck=50, six=True)
-    assert sa == sb == sc == 0 and ia == ib == ic and np.array_equal(Ca, Cb) and np.array_equal(Ca, Cc)
+    # voxel noise with void and fluid cells: some load cases stop on a rule, others at maxiter -- the same way in all three calls
+    Ca, ia, sa = gpu.solve_image_host(K, G, tol=1e-6, maxiter=1500, ncheck=50)
+    Cb, ib, sb = gpu.solve_image_host_segmented(ph, Kt, Gt, tol=1e-6, maxiter=1500, ncheck=50)
+    Cc, ic, sc = gpu.solve_image_host_segmented(ph, Kt, Gt, tol=1e-6, maxiter=1500, ncheck=50, six=True)
+    assert sa == sb == sc and sa in (0, gpu.MAXITER) and ia == ib == ic and np.array_equal(Ca, Cb) and np.array_equal(Ca, Cc)
     with pytest.raises(gpu.DrError) as e:                 # an id beyond the table
         gpu.Solver(Kt[:4], Gt[:4], phase=torch.from_numpy(ph).cuda())
     assert e.value.status == gpu.ERR_ARG
