@@ -215,7 +215,7 @@ def main():
     ap.add_argument("--form", type=int, default=0, help="0 stress-relaxation form of the paper (default, 160 B/voxel), 1 displacement form (112 B/voxel)")
     ap.add_argument("--palette", type=int, default=1, help="1 (default): uint8 phase ids + table when the image has <= 256 distinct (K,G); 0: fp64 modulus fields")
     ap.add_argument("--cpu-sample-n", type=int, default=191)
-    ap.add_argument("--cpu-iters", type=int, default=100)
+    ap.add_argument("--cpu-iters", type=int, default=600, help="oracle PT iterations of the cpu_baseline sample (~13 s on 16 cores at 191^3)")
     ap.add_argument("--cpu-iters-per-step", type=int, default=5)
     ap.add_argument("--cpu-threads", type=int, default=0, help="--impl reference: OMP_NUM_THREADS of the oracle (0 = all host cores)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
