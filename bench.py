@@ -222,6 +222,7 @@ def main():
     ap.add_argument("--e2e-iters", type=int, default=50, help="PT iterations per load case in the host-buffer e2e call")
     ap.add_argument("--time-to-solution", action="store_true", help="also solve all six load cases to tol 1e-8")
     ap.add_argument("--tol", type=float, default=1e-8)
+    ap.add_argument("--direct-offdiag", action="store_true", help="time-to-solution: also run the 7th (triaxial) test and report Eq. 27-29")
     ap.add_argument("--st-factor", type=float, default=1.0, help="DR_ST_FACTOR (non-default tuning: 0.7 needs ~35 %% fewer iterations at 479^3)")
     ap.add_argument("--void-rel", type=float, default=0.0, help="DR_VOID_REL (non-default: exact-void clamp of near-void cells)")
     ap.add_argument("--tts-maxiter-n", type=int, default=100, help="time-to-solution: maxiter = this x n per load case")
@@ -371,6 +372,14 @@ def main():
                    "params": dict(extra, form=args.form, kernel=args.kernel), "stop": [int(l[4]) for l in log] if len(log[0]) > 4 else None,
                    "iters": [l[1] for l in log], "status": [l[0] for l in log], "residual": [l[2] for l in log],
                    "C": [[float("%.6f" % v) for v in row] for row in C]}
+            if args.direct_offdiag:
+                # the paper's 7th direct test (App. A.3): load case 6 + Eq. 27-29 against the symmetrised columns of C
+                st7 = s.solve(6, args.eps0, args.tol, args.tts_maxiter_n * n)
+                d7 = s.offdiag_direct()
+                sym = [0.5 * (C[0, 1] + C[1, 0]), 0.5 * (C[0, 2] + C[2, 0]), 0.5 * (C[1, 2] + C[2, 1])]
+                tts["direct_offdiag"] = {"status": int(st7), "iters": s.info()[0], "C12_C13_C23": [float(v) for v in d7],
+                                         "symmetrised_columns": [float(v) for v in sym],
+                                         "max_abs_diff": float(max(abs(a - b) for a, b in zip(d7, sym)))}
             # the same six columns with all load cases in every launch (dr_solve_all) where six state
             # sets fit the device; timed from dr_create to the 6x6 read-back, second of two calls (the first warms up)
             need6 = binding.workspace_bytes(n, n, n, True)
