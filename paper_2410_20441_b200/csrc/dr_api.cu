@@ -72,6 +72,7 @@ struct dr_handle {
     unsigned long long* codes;  // [nz+5][gy2][gx2][TB2_TY][TB2_TX]
     unsigned long long *ekeys, *rkeys;   // edge-modulus and 1/H_node tables (bit patterns), 256 each
     double* tabs;               // TB2_TAB_N table values
+    double tabs_host[TB2_TAB_N];   // host copy (the derived tables of a launch are formed from it, TB2_CTAB)
     bool has_codes;             // codes and tables are valid for (code_gavg, code_void)
     bool codes_failed;          // more than 256 distinct edge / node values for that setting: one-sweep kernel instead
     int code_gavg; double code_void;
@@ -465,6 +466,7 @@ static dr_status ensure_codes(dr_handle* H) {
 #undef DR_CODE
     k_code_tables<<<1, 256, 0, H->st>>>(H->pal, H->ekeys, H->rkeys, H->tabs);
     CKL("k_code_tables");
+    CK(cudaMemcpyAsync(H->tabs_host, H->tabs, TB2_TAB_N * sizeof(double), cudaMemcpyDeviceToHost, H->st));
     CK(cudaMemcpyAsync(&fl, H->flags, 4, cudaMemcpyDeviceToHost, H->st));
     CK(cudaStreamSynchronize(H->st));
     if (fl & 16u) return fail(H, DR_ERR_CUDA, "stencil code lookup missed a table entry (internal error)");
@@ -525,6 +527,22 @@ static dr_status launch_coded(dr_handle* H, DrTb2Batch& TB, int nslots, bool wit
     TB.fs = H->buf[0][1] - H->buf[0][0];
     TB.codes = H->codes; TB.tabs = H->tabs; TB.gx = (int)grd.x; TB.gy = (int)grd.y; TB.nchunks = nchunks;
     TB.l2_hint = 0x1000000000000000ull;
+#if TB2_CTAB
+    {
+        // derived tables (TB2_S_*): the same expressions, in the same order, the kernel used to evaluate per CTA; theta, h and
+        // C~ are those of the handle, hence equal for every slot of a batch
+        const DrPT& P0 = TB.P[0];
+        const double thh = P0.theta * P0.inv_h, cvh = P0.c2t * P0.inv_h;
+        for (int e = 0; e < 256; ++e) {
+            const double Kv = H->tabs_host[TB2_TAB_K + e], Gv = H->tabs_host[TB2_TAB_G + e], Rv = H->tabs_host[TB2_TAB_R + e];
+            TB.dtab[TB2_S_LAM + e] = std::fma(-(2.0 / 3.0), Gv, Kv);
+            TB.dtab[TB2_S_G2 + e] = 2.0 * Gv;
+            TB.dtab[TB2_S_ES + e] = thh * H->tabs_host[TB2_TAB_E + e];
+            TB.dtab[TB2_S_CV + e] = cvh * Rv;
+            TB.dtab[TB2_S_RH + e] = Rv;
+        }
+    }
+#endif
     const size_t smem = DrTb2Cfg<TB2_TX, TB2_TY>::SMEM;
     if (nit == 2) { if (with_res) k_pt_tb2<1, 2, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(TB, H->L, lz);
                     else          k_pt_tb2<0, 2, TB2_TX, TB2_TY><<<grd, blk, smem, H->st>>>(TB, H->L, lz); }

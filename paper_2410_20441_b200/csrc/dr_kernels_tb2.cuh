@@ -50,6 +50,10 @@
 #ifndef TB2_LG128
 #define TB2_LG128 0        // 1: lambda and 2G of a cell come with one 16-byte table read
 #endif
+#ifndef TB2_CTAB
+#define TB2_CTAB 1         // 1: the derived tables travel in the kernel parameters and are read with LDC (constant cache, indexed per
+                           //    thread) instead of from shared memory: 16 table reads per thread and step leave the shared-memory pipe
+#endif
 #define TB2_KLO 2          // coded layers below layer 0 (layers -2, -1) ...
 #define TB2_KHI 3          // ... and above layer nz-1 (layers nz, nz+1, nz+2)
 
@@ -60,7 +64,8 @@
 #define TB2_TAB_E 512
 #define TB2_TAB_R 768
 #define TB2_TAB_N 1024
-// what a CTA derives from them once, in shared memory: the products that are the same in every iteration
+// the derived tables (TB2_CTAB: formed on the host per launch and passed in the kernel parameters, read with per-thread
+// indexed LDC; else built by every CTA in shared memory): the products that are the same in every iteration
 //   LAM = K - 2G/3,  G2 = 2G (interleaved, entry e at 2e and 2e+1, when TB2_LG128),  ES = (theta/h) E,  CV = (C~^2 h^2 / (theta h)) R,  RH = R (residual launches only)
 #define TB2_S_LAM 0
 #define TB2_S_G2 256
@@ -81,6 +86,9 @@ struct DrTb2Batch {
     const double* tabs;                   // TB2_TAB_N doubles
     int gx, gy, nchunks;
     unsigned long long l2_hint;
+#if TB2_CTAB
+    double dtab[1280];                    // derived tables TB2_S_* (LAM G2 ES CV RH), formed on the host from tabs
+#endif
 };
 // what the march needs of one slot
 struct DrTb2Maps {
@@ -168,14 +176,21 @@ __device__ __forceinline__ DrStress6 dr_tb2_stress(const DrPT& P, const int nx, 
     return n;
 }
 
+// entry of derived table SEC (TB2_S_*) at byte offset off8 = 8 x index
+#if TB2_CTAB
+#define TB2_TAB(SEC, off8) (*reinterpret_cast<const double*>(reinterpret_cast<const char*>(TB.dtab + (SEC)) + (off8)))
+#else
+#define TB2_TAB(SEC, off8) (*reinterpret_cast<const double*>(reinterpret_cast<const char*>(tab + (SEC)) + (off8)))
+#endif
+
 // velocity update of one node (Eq. 11): v += C~^2 h^2 / (theta H_node) F, with F = Fh / h the stress divergence;
 // cv = C~^2 h^2 / (theta h H_node) and rH = 1/H_node from the tables, both 0 for wall, dead and out-of-domain nodes
 // (never updated, not part of the residual).  rmax collects |Fh| / H_node (scaled by 1/h and h/|eps0| at the end).
 template <int RES>
-__device__ __forceinline__ double dr_tb2_vel(const double v, const double Fh, const double* tab, const unsigned idx8, double& rmax, bool& rnan) {
-    const double cv = *reinterpret_cast<const double*>(reinterpret_cast<const char*>(tab + TB2_S_CV) + idx8);
+__device__ __forceinline__ double dr_tb2_vel(const double v, const double Fh, const DrTb2Batch& TB, const double* tab, const unsigned idx8, double& rmax, bool& rnan) {
+    const double cv = TB2_TAB(TB2_S_CV, idx8);
     if (RES) {
-        const double r = fabs(Fh) * *reinterpret_cast<const double*>(reinterpret_cast<const char*>(tab + TB2_S_RH) + idx8);
+        const double r = fabs(Fh) * TB2_TAB(TB2_S_RH, idx8);
         if (cv != 0.0) { rnan |= !(r == r); rmax = dr_max(rmax, r); }
     }
     return cv != 0.0 ? fma(cv, Fh, v) : v;
@@ -190,12 +205,12 @@ __device__ __forceinline__ double dr_tab_at(const double* tab, const unsigned of
 }
 
 // lambda = K - 2G/3 and 2G of the cell whose table offset (index x 8) is off8
-__device__ __forceinline__ void dr_tab_lg(const double* tab, const unsigned off8, double& lam, double& g2) {
-#if TB2_LG128
+__device__ __forceinline__ void dr_tab_lg(const DrTb2Batch& TB, const double* tab, const unsigned off8, double& lam, double& g2) {
+#if TB2_LG128 && !TB2_CTAB
     const double2 v = *reinterpret_cast<const double2*>(reinterpret_cast<const char*>(tab) + 2u * off8);    // interleaved: one 16-byte read
     lam = v.x; g2 = v.y;
 #else
-    lam = dr_tab_at(tab + TB2_S_LAM, off8); g2 = dr_tab_at(tab + TB2_S_G2, off8);
+    lam = TB2_TAB(TB2_S_LAM, off8); g2 = TB2_TAB(TB2_S_G2, off8);
 #endif
 }
 
@@ -233,7 +248,7 @@ struct DrTb2Out { double* col; long long fs; };
 // thread's own address: the compiler can then interleave the four stages freely.
 // code2: in = stencil code of layer k-2 (stored by step t-2, same parity), out = that of layer k.
 template <int RES, int NIT, int TX, int TY, bool BND, int Q>
-__device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, const DrTb2Maps& T, const DrTb2Out& g,
+__device__ __forceinline__ void dr_tb2_step(const DrTb2Batch& TB, const DrLayout& L, const DrPT& P, const DrTb2Maps& T, const DrTb2Out& g,
                                             double* sm, const double* tab, const unsigned long long* codesrc, const long long codestride,
                                             unsigned long long* bars, const int s, const int t, const int k,
                                             const int kb, const int ke, const int i, const int j, const int x0, const int y0,
@@ -264,9 +279,9 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
         o.sxx = X1p[Y_SXX * PL]; o.syy = X1p[Y_SYY * PL]; o.szz = X1p[Y_SZZ * PL];
         o.txy = X1p[Y_TXY * PL]; o.txz = X1p[Y_TXZ * PL]; o.tyz = X1p[Y_TYZ * PL];
         double lam2, g22;
-        dr_tab_lg(tab, dr_code_off(c2, 0), lam2, g22);
+        dr_tab_lg(TB, tab, dr_code_off(c2, 0), lam2, g22);
         const DrStress6 m2 = dr_tb2_stress<BND>(P, nx, ny, nz, i, j, k2, lam2, g22,
-                                dr_tab_at(tab + TB2_S_ES, dr_code_off(c2, 1)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c2, 2)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c2, 3)),
+                                TB2_TAB(TB2_S_ES, dr_code_off(c2, 1)), TB2_TAB(TB2_S_ES, dr_code_off(c2, 2)), TB2_TAB(TB2_S_ES, dr_code_off(c2, 3)),
                                 V1c[0 * PL], V1c[1 * PL], V1c[2 * PL], V1c[0 * PL + 1], V1c[1 * PL + TX], V1c[0 * PL - TX], V1c[1 * PL - 1],
                                 V1n[0 * PL], V1n[1 * PL], V1n[2 * PL], V1n[2 * PL - 1], V1n[2 * PL - TX], o);
         X2p[Z_SXX * PL] = m2.sxx; X2p[Z_SYY * PL] = m2.syy; X2p[Z_TXY * PL] = m2.txy;
@@ -287,9 +302,9 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
         DrStress6 o;
         o.sxx = Bs[0 * PL]; o.syy = Bs[1 * PL]; o.szz = Bs[2 * PL]; o.txy = Bs[3 * PL]; o.txz = Bs[4 * PL]; o.tyz = Bs[5 * PL];
         double lam1, g21;
-        dr_tab_lg(tab, dr_code_off(c1, 0), lam1, g21);
+        dr_tab_lg(TB, tab, dr_code_off(c1, 0), lam1, g21);
         m1 = dr_tb2_stress<BND>(P, nx, ny, nz, i, j, k, lam1, g21,
-                                dr_tab_at(tab + TB2_S_ES, dr_code_off(c1, 1)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c1, 2)), dr_tab_at(tab + TB2_S_ES, dr_code_off(c1, 3)),
+                                TB2_TAB(TB2_S_ES, dr_code_off(c1, 1)), TB2_TAB(TB2_S_ES, dr_code_off(c1, 2)), TB2_TAB(TB2_S_ES, dr_code_off(c1, 3)),
                                 vxc, vyc, vzc, Ac[0 * PL + 1], Ac[1 * PL + TX], Ac[0 * PL - TX], Ac[1 * PL - 1],
                                 An[0 * PL], An[1 * PL], An[2 * PL], An[2 * PL - 1], An[2 * PL - TX], o);
         // X1p held layer k-2 (read above by this same thread): now layer k
@@ -321,12 +336,12 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
             if (ck) {
                 if (cj) {                           // v_x at (i, j+1/2, k2+1/2)
                     const double Fx = (msxx - Z[Z_SXX * PL - 1]) + (Z[Z_TXY * PL + TX] - mtxy) + (gn.txz - gc.txz);
-                    po[F_VX * g.fs] = dr_tb2_vel<RES>(V1c[0 * PL], Fx, tab, dr_code_off(c2, 4), rmax, rnan);
+                    po[F_VX * g.fs] = dr_tb2_vel<RES>(V1c[0 * PL], Fx, TB, tab, dr_code_off(c2, 4), rmax, rnan);
                     po[F_TXZ * g.fs] = gc.txz;
                 }
                 if (ci) {                           // v_y at (i+1/2, j, k2+1/2)
                     const double Fy = (Z[Z_TXY * PL + 1] - mtxy) + (msyy - Z[Z_SYY * PL - TX]) + (gn.tyz - gc.tyz);
-                    po[F_VY * g.fs] = dr_tb2_vel<RES>(V1c[1 * PL], Fy, tab, dr_code_off(c2, 5), rmax, rnan);
+                    po[F_VY * g.fs] = dr_tb2_vel<RES>(V1c[1 * PL], Fy, TB, tab, dr_code_off(c2, 5), rmax, rnan);
                     po[F_TYZ * g.fs] = gc.tyz;
                 }
                 po[F_TXY * g.fs] = mtxy;
@@ -337,7 +352,7 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
             }
             if (ci && cj) {                         // v_z at (i+1/2, j+1/2, k2)
                 const double Fz = (gc.txz_r - gc.txz) + (gc.tyz_u - gc.tyz) + (gn.szz - gc.szz);
-                po[F_VZ * g.fs] = dr_tb2_vel<RES>(V1c[2 * PL], Fz, tab, dr_code_off(c2, 6), rmax, rnan);
+                po[F_VZ * g.fs] = dr_tb2_vel<RES>(V1c[2 * PL], Fz, TB, tab, dr_code_off(c2, 6), rmax, rnan);
             }
         }
     }
@@ -351,23 +366,23 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
             const double Fy = (Y[Y_TXY * PL + 1] - m1.txy) + (m1.syy - Y[Y_SYY * PL - TX]) + (m1.tyz - fc.tyz);
             const double Fz = (fc.txz_r - fc.txz) + (fc.tyz_u - fc.tyz) + (m1.szz - fc.szz);
             if (NIT == 2) {
-                nvx = dr_tb2_vel<0>(vxc, Fx, tab, dr_code_off(c1, 4), r1, n1);
-                nvy = dr_tb2_vel<0>(vyc, Fy, tab, dr_code_off(c1, 5), r1, n1);
-                nvz = dr_tb2_vel<0>(vzc, Fz, tab, dr_code_off(c1, 6), r1, n1);
+                nvx = dr_tb2_vel<0>(vxc, Fx, TB, tab, dr_code_off(c1, 4), r1, n1);
+                nvy = dr_tb2_vel<0>(vyc, Fy, TB, tab, dr_code_off(c1, 5), r1, n1);
+                nvz = dr_tb2_vel<0>(vzc, Fz, TB, tab, dr_code_off(c1, 6), r1, n1);
             } else if (row2 && in2 && k >= kb) {    // NIT == 1: a plain one-iteration sweep on the same geometry
                 double* const po = g.col + sz * k;
                 const bool ck = k < nz;
                 const bool ci = !BND || i < nx, cj = !BND || j < ny;
                 if (ck) {
-                    if (cj) { po[F_VX * g.fs] = dr_tb2_vel<RES>(vxc, Fx, tab, dr_code_off(c1, 4), rmax, rnan); po[F_TXZ * g.fs] = fc.txz; }
-                    if (ci) { po[F_VY * g.fs] = dr_tb2_vel<RES>(vyc, Fy, tab, dr_code_off(c1, 5), rmax, rnan); po[F_TYZ * g.fs] = fc.tyz; }
+                    if (cj) { po[F_VX * g.fs] = dr_tb2_vel<RES>(vxc, Fx, TB, tab, dr_code_off(c1, 4), rmax, rnan); po[F_TXZ * g.fs] = fc.txz; }
+                    if (ci) { po[F_VY * g.fs] = dr_tb2_vel<RES>(vyc, Fy, TB, tab, dr_code_off(c1, 5), rmax, rnan); po[F_TYZ * g.fs] = fc.tyz; }
                     po[F_TXY * g.fs] = m1.txy;
                     if (ci && cj) { po[F_SXX * g.fs] = m1.sxx; po[F_SYY * g.fs] = m1.syy; po[F_SZZ * g.fs] = m1.szz; }
                 } else {
                     if (cj) po[F_TXZ * g.fs] = fc.txz;
                     if (ci) po[F_TYZ * g.fs] = fc.tyz;
                 }
-                if (ci && cj) po[F_VZ * g.fs] = dr_tb2_vel<RES>(vzc, Fz, tab, dr_code_off(c1, 6), rmax, rnan);
+                if (ci && cj) po[F_VZ * g.fs] = dr_tb2_vel<RES>(vzc, Fz, TB, tab, dr_code_off(c1, 6), rmax, rnan);
             }
         }
         if (NIT == 2) { V1c[0 * PL] = nvx; V1c[1 * PL] = nvy; V1c[2 * PL] = nvz; }   // layer k replaces layer k-2 (read above)
@@ -376,7 +391,7 @@ __device__ __forceinline__ void dr_tb2_step(const DrLayout& L, const DrPT& P, co
 }
 
 template <int RES, int NIT, int TX, int TY, bool BND>
-__device__ __forceinline__ void dr_tb2_march(const DrLayout& L, const DrPT& P, const DrTb2Maps& T, const DrTb2Out& g,
+__device__ __forceinline__ void dr_tb2_march(const DrTb2Batch& TB, const DrLayout& L, const DrPT& P, const DrTb2Maps& T, const DrTb2Out& g,
                                              double* sm, const double* tab, const unsigned long long* codesrc, const long long codestride,
                                              unsigned long long* bars, const int s, const int kb, const int ke,
                                              const int i, const int j, const int x0, const int y0,
@@ -388,7 +403,7 @@ __device__ __forceinline__ void dr_tb2_march(const DrLayout& L, const DrPT& P, c
     const int klast = ke + (NIT == 2 ? 1 : -1);               // last step: second iteration of layer ke-1
     int k = kb - 2;
 #define DR_TB2_STEP(Q_, FC, FN, GC, GN, CC) \
-    dr_tb2_step<RES, NIT, TX, TY, BND, Q_>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, t + Q_, k + Q_, kb, ke, i, j, x0, y0, producer, in1, row1, row2, in2, FC, FN, GC, GN, CC, rmax, rnan)
+    dr_tb2_step<RES, NIT, TX, TY, BND, Q_>(TB, L, P, T, g, sm, tab, codesrc, codestride, bars, s, t + Q_, k + Q_, kb, ke, i, j, x0, y0, producer, in1, row1, row2, in2, FC, FN, GC, GN, CC, rmax, rnan)
 #if TB2_UNROLL4
     for (int t = 0; k <= klast; t += 4, k += 4) {
         DR_TB2_STEP(0, fa, fb, ga, gb, ca);
@@ -412,7 +427,11 @@ __global__ void __launch_bounds__(TX * TY, 1)
 k_pt_tb2(const __grid_constant__ DrTb2Batch TB, DrLayout L, int lz) {
     extern __shared__ __align__(1024) double sm[];
     __shared__ __align__(8) unsigned long long bars[4];
+#if TB2_CTAB
+    const double* const tab = nullptr;                        // tables: TB.dtab, read with LDC
+#else
     __shared__ __align__(16) double tab[RES ? 1280 : 1024];
+#endif
     using Cfg = DrTb2Cfg<TX, TY>;
     constexpr int PL = Cfg::PL;
     const int nx = L.nx, ny = L.ny, nz = L.nz;
@@ -431,6 +450,7 @@ k_pt_tb2(const __grid_constant__ DrTb2Batch TB, DrLayout L, int lz) {
     const unsigned long long* codesrc = TB.codes + ((long long)blockIdx.y * TB.gx + blockIdx.x) * PL;
     const int s = ty * TX + tx;
     // derived tables (see TB2_S_*): the products that do not change from one iteration to the next
+#if !TB2_CTAB
     {
         const double thh = P.theta * P.inv_h, cvh = P.c2t * P.inv_h;
         for (int e = s; e < 256; e += TX * TY) {
@@ -442,6 +462,7 @@ k_pt_tb2(const __grid_constant__ DrTb2Batch TB, DrLayout L, int lz) {
             if (RES) tab[TB2_S_RH + e] = Rv;
         }
     }
+#endif
     const bool producer = (tx == 0 && ty == 0);
     const bool in1 = tx >= 1 && tx <= TX - 2 && ty >= 1 && ty <= TY - 2;
     const bool row1 = ty >= 1 && ty <= TY - 2;
@@ -469,8 +490,8 @@ k_pt_tb2(const __grid_constant__ DrTb2Batch TB, DrLayout L, int lz) {
     bool rnan = false;
     // extended tile free of boundary nodes?
     const bool interior = ib >= 1 && ib + TX - 1 <= nx - 1 && jb >= 1 && jb + TY - 1 <= ny - 1;
-    if (interior) dr_tb2_march<RES, NIT, TX, TY, false>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row1, row2, in2, rmax, rnan);
-    else          dr_tb2_march<RES, NIT, TX, TY, true>(L, P, T, g, sm, tab, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row1, row2, in2, rmax, rnan);
+    if (interior) dr_tb2_march<RES, NIT, TX, TY, false>(TB, L, P, T, g, sm, tab, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row1, row2, in2, rmax, rnan);
+    else          dr_tb2_march<RES, NIT, TX, TY, true>(TB, L, P, T, g, sm, tab, codesrc, codestride, bars, s, kb, ke, i, j, x0, y0, producer, in1, row1, row2, in2, rmax, rnan);
 
     if (RES) {
         __shared__ unsigned long long smr[32];
