@@ -95,7 +95,7 @@ typedef enum {
 size_t dr_workspace_bytes(int nx, int ny, int nz);
 
 /* Bytes of device workspace for a handle that can also run dr_solve_all: six state sets instead of one (0 if the sizes are
- * invalid).  191^3: 7.4 GB, 479^3: 111 GB, 703^3 does not fit one B200 -- the batch is meant for small and medium grids. */
+ * invalid).  191^3: 7.7 GB, 479^3: 111.5 GB, 703^3 does not fit one B200 -- the batch is meant for small and medium grids. */
 size_t dr_workspace_bytes_six(int nx, int ny, int nz);
 
 /* Create a solver.  nx,ny,nz >= 2; h > 0.
