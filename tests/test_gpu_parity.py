@@ -504,3 +504,16 @@ def test_segmented_create_is_bitwise_the_fp64_create(oracle_mod, gpu):
     with pytest.raises(gpu.DrError) as e:                 # negative modulus in the table
         gpu.Solver(np.array([1.0, -1.0, 1.0, 1.0, 1.0]), Gt, phase=torch.from_numpy(ph).cuda())
     assert e.value.status == gpu.ERR_ARG
+
+
+# ------------------------------------------------------------------------------------------------ maximum extent per axis
+@pytest.mark.parametrize("shape", [(8192, 2, 2), (2, 8192, 3), (3, 2, 8192)])
+def test_maximum_extent_along_one_axis(oracle_mod, gpu, shape):
+    """the largest size dr.h admits (8192) along x, y and z in turn, two or three nodes across: hundreds of tiles / z chunks
+    of mostly halo; coded two-iteration kernel and the one-sweep kernel against the oracle, shear and normal load case"""
+    K, G = _quantised(shape, 3, seed=shape[0] + 2 * shape[1])
+    for kernel, lc, n in ((3, 2, 5), (3, 4, 4), (0, 5, 3)):
+        errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, lc, 1e-4, n, kernel=kernel)
+        assert max(errs) <= FIELD_TOL, (kernel, lc, errs)
+        assert abs(ro - rs) <= 1e-9 * ro
+    assert gpu.workspace_bytes(8193, 2, 2) == 0
