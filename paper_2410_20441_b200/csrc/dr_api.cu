@@ -494,7 +494,7 @@ static dr_status prepare(dr_handle* H, int lc, double eps0) {
     const DrLayout& L = H->L;
     { dr_status ms = prepare_moduli(H); if (ms != DR_OK) return ms; }
     DrPT P = make_pt(H, lc, eps0);
-    dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
+    dim3 blk(32, 4, 1), grd(((L.nx + 3) / 2 + 31) / 32, (L.ny + 1 + 3) / 4, (L.nz + 1 + DR_BC_ZB - 1) / DR_BC_ZB);   // pairs (2t-1, 2t), t = 0 .. (nx+2)/2
     if (H->form == 1 && H->kernel == 2) return fail(H, DR_ERR_ARG, "DR_FORM = 1 is implemented by DR_KERNEL 0 and 1 only");
     if (H->gavg) k_bc_init<1><<<grd, blk, 0, H->st>>>(H->L, P, fields_of(H, 0), fields_of(H, 1), H->form, H->K, H->G);
     else         k_bc_init<0><<<grd, blk, 0, H->st>>>(H->L, P, fields_of(H, 0), fields_of(H, 1), H->form, H->K, H->G);
@@ -868,7 +868,7 @@ extern "C" dr_status dr_solve_all(dr_handle* H, double eps0, double tol, int max
     for (int lc = 0; lc < 6; ++lc) {
         P[lc] = make_pt(H, lc, eps0);
         DrFields F; for (int f = 0; f < F_COUNT; ++f) F.f[f] = H->xbuf[lc][0][f];
-        dim3 blk(64, 4, 1), grd((L.nx + 1 + 63) / 64, (L.ny + 1 + 3) / 4, L.nz + 1);
+        dim3 blk(32, 4, 1), grd(((L.nx + 3) / 2 + 31) / 32, (L.ny + 1 + 3) / 4, (L.nz + 1 + DR_BC_ZB - 1) / DR_BC_ZB);   // pairs (2t-1, 2t), t = 0 .. (nx+2)/2
         if (H->gavg) k_bc_init<1><<<grd, blk, 0, H->st>>>(H->L, P[lc], F, F, 0, H->K, H->G);
         else         k_bc_init<0><<<grd, blk, 0, H->st>>>(H->L, P[lc], F, F, 0, H->K, H->G);
         CKL("k_bc_init");
