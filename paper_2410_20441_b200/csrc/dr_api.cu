@@ -519,7 +519,7 @@ static void fill_slot(dr_handle* H, DrTb2Batch& TB, int slot, int set, int cur, 
 static dr_status launch_coded(dr_handle* H, DrTb2Batch& TB, int nslots, bool with_res, int nit) {
     const DrLayout& L = H->L;
     // a batch of load cases multiplies the CTA count: pick the z chunk that fills whole waves for THIS number of slots
-    // (small grids: 32^3 runs 2-layer chunks alone and 11-layer chunks with six load cases; results do not depend on it)
+    // (small grids: 32^3 runs 2-layer chunks alone and 9-layer chunks with six load cases; results do not depend on it)
     const int lz = (H->lz_user || nslots == 1) ? H->tb2_lz
                                                : choose_lz_for(tb2_tiles_x(L) * tb2_tiles_y(L) * nslots, L.nz + 1, 4, DR_LZ_MAX_TB2);
     const int nchunks = (L.nz + 1 + lz - 1) / lz;
