@@ -177,6 +177,44 @@ dr_status dr_offdiag_direct(dr_handle* h, double out[3]);
 /* Volume-averaged stresses of the last solve/step, HOST pointer, Voigt order (Eq. 7). */
 dr_status dr_avg_stress(dr_handle* h, double out[6]);
 
+/* Volume-averaged stresses (Eq. 7, Reading R7: cell sum of the normal stresses, trapezoid weights on the edge shears)
+ * of six DENSE device fields, WITHOUT a handle, a workspace or any allocation.
+ *
+ * Why it exists.  Every other compute call works in a workspace the caller allocated.  Some callers have no way to get
+ * one: a progress or post-processing hook running beside a long solve, where a cudaMalloc / cudaFree would serialise
+ * against all work on the device and stall the solver's streams each time; or a plug-in inside a host program whose
+ * allocator already holds whatever device memory a large image leaves free, so that an allocation of the plug-in's own
+ * fails.  For them the reduction scratch is a fixed 6 MiB array compiled into libdr.so itself.  Every GPU on which the
+ * library's device code gets loaded carries these 6 MiB until the process exits, whether or not this call is ever used.
+ *
+ * Arguments.  stress: HOST array of six DEVICE pointers in Voigt order, each a dense x-fastest array as dr_get_field
+ * writes it: sxx, syy, szz (nx,ny,nz), tyz (nx,ny+1,nz+1), txz (nx+1,ny,nz+1), txy (nx+1,ny+1,nz); read only, borrowed until
+ * the work enqueued by this call has run.  out6: DEVICE, 6 doubles, written by the last kernel of the call.  cuda_stream:
+ * cudaStream_t or NULL; both kernels go there and the call does NOT synchronise -- read out6 in stream order.  All pointers
+ * and the stream belong to the CURRENT device (there is no handle to remember one).  errbuf: HOST, errbuf_len bytes, or
+ * NULL; receives a message whenever the return value is not DR_OK (emptied on success).
+ *
+ * Limit.  (ny+1)*(nz+1) <= DR_STATIC_MAX_ROWS (the scratch holds six partial sums per eight x-rows); nx, ny, nz in 2..8192.
+ * That covers every cube up to 1023^3 (all five benchmark images).  A larger grid is refused with DR_ERR_ARG and a message
+ * that names the limit; nothing is launched.  Use a handle and dr_avg_stress there.
+ *
+ * First call.  The first call on each device looks up that device's address of the built-in array
+ * (cudaGetSymbolAddress, checked; DR_ERR_CUDA if it fails) and keeps it for the process.  Make that first call during
+ * set-up, before any stream capture is begun.  Later calls only launch two kernels.  No cudaMalloc, cudaFree, host
+ * allocation or allocating library routine is called on any path.
+ *
+ * Sharing.  There is ONE array per device and every call uses it.  It is not cleared: a call overwrites the part it will
+ * read, so nothing has to start at zero and whatever an earlier call left is never looked at.  Two calls whose kernels can
+ * overlap on the GPU (different streams, or different host threads on different streams) write the same partial sums and
+ * both results are then garbage -- keep all calls on one stream, or order them with events.
+ *
+ * Result.  Same weights and the same quantity as dr_avg_stress after dr_step / dr_solve on the fields of that handle; the sum is
+ * grouped differently (by eight rows instead of by a fixed number of blocks), so the two agree to rounding, not bit for
+ * bit.  Run-to-run deterministic.  Without a CUDA device: DR_ERR_CUDA. */
+#define DR_STATIC_MAX_ROWS 1048576
+dr_status dr_avg_stress_static(int nx, int ny, int nz, const double* const stress[6], double* out6,
+                               void* cuda_stream, char* errbuf, size_t errbuf_len);
+
 /* Iterations done, last residual, and milliseconds (CUDA events on the stream, whole call) of the last
  * dr_solve/dr_step.  Any pointer may be NULL. */
 dr_status dr_info(dr_handle* h, int* iters, double* residual, double* ms);

@@ -19,7 +19,8 @@ PARAM_IDS = dict(cfl=CFL, st_factor=ST_FACTOR, ncheck=NCHECK, gavg=GAVG, void_re
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "tyz", "txz", "txy")
 EXPORTS = ("dr_workspace_bytes", "dr_workspace_bytes_six", "dr_solve_all", "dr_info_lc", "dr_create", "dr_create_segmented", "dr_solve_image_host_segmented", "dr_set_param", "dr_solve", "dr_solve_six", "dr_effective_C_six", "dr_step", "dr_iterate",
            "dr_effective_C", "dr_avg_stress", "dr_offdiag_direct", "dr_info", "dr_get_field", "dr_solve_image_host", "dr_contribution_tensor",
-           "dr_uses_palette", "dr_active_kernel", "dr_stop_reason", "dr_launch_count", "dr_last_error", "dr_destroy")
+           "dr_uses_palette", "dr_active_kernel", "dr_stop_reason", "dr_launch_count", "dr_last_error", "dr_destroy", "dr_avg_stress_static")
+STATIC_MAX_ROWS = 1048576          # DR_STATIC_MAX_ROWS of include/dr.h
 
 _lib = None
 
@@ -68,6 +69,8 @@ def lib():
             L.dr_active_kernel.argtypes = [vp]
         if hasattr(L, "dr_stop_reason"):
             L.dr_stop_reason.argtypes = [vp]
+        if hasattr(L, "dr_avg_stress_static"):
+            L.dr_avg_stress_static.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(vp), vp, vp, C.c_char_p, C.c_size_t]
         L.dr_launch_count.argtypes = [vp]
         L.dr_launch_count.restype = C.c_longlong
         L.dr_last_error.argtypes = [vp]
@@ -237,6 +240,36 @@ class Solver:
             self.close()
         except Exception:
             pass
+
+
+def avg_stress_static(fields, out=None, stream=None):
+    """dr_avg_stress_static: <sigma> (Eq. 7) of six dense stress fields with no handle, no workspace and no allocation inside the
+    library -- for callers that cannot allocate device memory (a hook beside a running solve, where cudaMalloc would stall the
+    device; a plug-in whose host owns the free memory).  The scratch is a 6 MiB array inside libdr.so, shared by all calls:
+    keep them on one stream.  Limit (ny+1)*(nz+1) <= STATIC_MAX_ROWS, else DrError(ERR_ARG) naming the limit.
+
+    fields: the six float64 CUDA tensors Solver.get_field(3..8) returns (sxx, syy, szz, tyz, txz, txy).  out: float64 CUDA
+    tensor of 6 elements; a caller that must not allocate passes its own (None: torch allocates one here, outside the library).
+    Enqueues on `stream` (default: torch's current stream) and does not synchronise; returns out."""
+    import torch
+    assert len(fields) == 6
+    nz, ny, nx = (int(s) for s in fields[0].shape)
+    for f, t in zip(range(3, 9), fields):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == field_shape(nx, ny, nz, f)):
+            raise TypeError("field %s must be a contiguous float64 CUDA tensor of shape %s" % (FIELDS[f], (field_shape(nx, ny, nz, f),)))
+    dev = fields[0].device
+    if out is None:
+        out = torch.empty(6, dtype=torch.float64, device=dev)
+    elif not (out.is_cuda and out.device == dev and out.dtype == torch.float64 and out.numel() == 6 and out.is_contiguous()):
+        raise TypeError("out must be a contiguous float64 tensor of 6 elements on the device of the fields")
+    ptrs = (C.c_void_p * 6)(*[t.data_ptr() for t in fields])
+    err = C.create_string_buffer(512)
+    with torch.cuda.device(dev):
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        rc = lib().dr_avg_stress_static(nx, ny, nz, ptrs, out.data_ptr(), st.cuda_stream, err, len(err))
+    if rc != OK:
+        raise DrError(rc, err.value.decode())
+    return out
 
 
 def contribution_tensor(C_eff, C_matrix, phi):

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdr.so")
-SOURCES = ["dr_api.cu"]
+SOURCES = ["dr_api.cu", "dr_static.cu"]      # dr_static.cu: dr_avg_stress_static, its own translation unit
 HEADERS = ["dr_layout.cuh", "dr_kernels_aux.cuh", "dr_kernels_split.cuh", "dr_kernels_fused.cuh", "dr_kernels_tma.cuh", "dr_kernels_tb2.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
