@@ -1,6 +1,9 @@
 // dr_api.cu -- host side of libdr: the C ABI of include/dr.h (handle, workspace carving, PT constants of
 // Eq. 14-21, iteration loop with periodic residual check, six-load-case bookkeeping).
-// All arithmetic of the method runs in the kernels of dr_kernels_*.cuh; there is no CPU fallback.
+// Every field update, residual and average of the method runs in the kernels of dr_kernels_*.cuh; there is no CPU fallback.
+// Host arithmetic is limited to scalars: the PT constants of Eq. 14-21 (make_pt), and, for the coded kernels, the <= 256-entry
+// derived tables of a launch (lambda = K - 2G/3, (theta/h) E, c^2/(theta h) R: launch_coded), formed from table values the
+// kernels k_code_tables / k_pal_values produced.
 #include <cuda_runtime.h>
 #include <cmath>
 #include <cstdio>
@@ -235,6 +238,8 @@ static void pinned_release(double* p) {
 // ~30 attribute calls are a visible part of dr_create on small grids
 static cudaError_t set_kernel_attributes(int device) {
     static bool done[64] = {false};
+    static std::mutex mu;                       // dr_create may be called from several host threads
+    std::lock_guard<std::mutex> lk(mu);
     if (device >= 0 && device < 64 && done[device]) return cudaSuccess;
     const cudaFuncAttribute A = cudaFuncAttributeMaxDynamicSharedMemorySize;
     const int smem = (int)DrFusedCfg<FUSED_TX, FUSED_TY>::SMEM;
@@ -446,7 +451,9 @@ static DrConstFields cfields_of(dr_handle* H, int b) {
 // more than 256 distinct (K,G) pairs, edge moduli or node stiffnesses is left uncoded (has_codes = false) and DR_KERNEL 3
 // then runs the one-sweep kernel
 static dr_status ensure_codes(dr_handle* H) {
-    if (!(H->has_pal && H->use_pal)) { H->has_codes = false; return DR_OK; }
+    // palette off: the codes are dropped, and so is their cache key -- switching DR_PALETTE back on must rebuild them instead
+    // of meeting the key below with has_codes still false (which left the handle on the one-sweep kernel)
+    if (!(H->has_pal && H->use_pal)) { H->has_codes = false; H->code_gavg = -1; return DR_OK; }
     if (H->code_gavg == H->gavg && H->code_void == H->void_applied) return DR_OK;      // built (or failed) for this setting
     const DrLayout& L = H->L;
     H->has_codes = false; H->codes_failed = false;
@@ -854,7 +861,14 @@ extern "C" dr_status dr_solve_all(dr_handle* H, double eps0, double tol, int max
             dr_status s = dr_solve(H, lc, eps0, tol, maxiter);
             H->lc_iters[lc] = H->iters; H->lc_res[lc] = H->residual; H->lc_stop[lc] = H->stop_reason;
             if (status_out) status_out[lc] = (int)s;
-            if (s != DR_OK && s != DR_MAXITER) return s;
+            if (s != DR_OK && s != DR_MAXITER) {
+                // hard error: the load cases that never ran report DR_ERR_STATE / no iterations instead of stale values
+                for (int m = lc + 1; m < 6; ++m) {
+                    H->lc_iters[m] = 0; H->lc_res[m] = INFINITY; H->lc_stop[m] = DR_STOP_NONE;
+                    if (status_out) status_out[m] = (int)DR_ERR_STATE;
+                }
+                return s;
+            }
             if (s == DR_MAXITER) worst = DR_MAXITER;
         }
         return worst;

@@ -158,6 +158,40 @@ def test_solve_all_batched_ragged_stagnation_maxiter_and_fallbacks(oracle_mod, g
     assert st == 0 and iters == [l[1] for l in logb] and np.array_equal(Ch, Cb)
 
 
+def test_palette_toggle_rebuilds_the_stencil_codes(gpu):
+    """DR_PALETTE 1 -> 0 -> 1 on one handle: the codes dropped at 0 are rebuilt at 1 (the cache key used to survive with
+    has_codes false, which left the handle on the one-sweep kernel until gavg or void_rel changed)"""
+    import torch
+    K, G = _quantised((40, 30, 20), 3, seed=3)
+    s = gpu.Solver(to_dev(K), to_dev(G))
+    s.step(2, 1e-4, 6)
+    assert s.active_kernel() == 3
+    f3 = _all_fields(s)
+    s.set_param("palette", 0)
+    s.step(2, 1e-4, 6)
+    assert s.active_kernel() == 0 and not s.uses_palette()
+    s.set_param("palette", 1)
+    s.step(2, 1e-4, 6)
+    assert s.active_kernel() == 3
+    for a, b in zip(f3, _all_fields(s)):
+        assert torch.equal(a, b)
+
+
+def test_solve_all_fallback_reports_every_load_case_after_a_hard_error(gpu):
+    """dr_solve_all on its six-plain-solves path (DR_KERNEL 0) with a C~ far above the stability limit: load case 0 diverges,
+    the call returns DR_ERR_DIVERGED, and the load cases that never ran say DR_ERR_STATE / 0 iterations / DR_STOP_NONE"""
+    import ctypes as C
+    K, G = _quantised((20, 18, 16), 3, seed=4)
+    b = gpu.Solver(to_dev(K), to_dev(G), six=True, kernel=0, cfl=3.0, ncheck=20)
+    stat = (C.c_int * 6)(*([-7] * 6))
+    rc = gpu.lib().dr_solve_all(b._h, 1e-4, 1e-8, 4000, stat)
+    assert rc == gpu.ERR_DIVERGED and list(stat) == [gpu.ERR_DIVERGED] + [gpu.ERR_STATE] * 5
+    for lc in range(1, 6):
+        it, r, sp = C.c_int(-1), C.c_double(-1.0), C.c_int(-1)
+        gpu.lib().dr_info_lc(b._h, lc, C.byref(it), C.byref(r), C.byref(sp))
+        assert it.value == 0 and sp.value == gpu.STOP_NONE and r.value == float("inf")
+
+
 def test_run_to_run_bitwise_determinism_and_kernel_equality_at_191(gpu):
     """compute-sanitizer's racecheck is not available on the GPU pool, so races in the shared-memory pipeline of the two-iteration
     kernel are hunted the other way: at 191^3 (560 CTAs of 512 threads, 4 waves, every tile shape) five runs of 60 iterations
