@@ -74,9 +74,12 @@ typedef enum {
     DR_STAG_TOL = 10,  /* second stopping rule of dr_solve (Reading R9b; the paper gives no rule beyond P:78): at every residual
                           check with res > tol the volume averages <sigma> (Eq. 7) are formed; two consecutive checks that
                           moved them by <= stag_tol (relative, max-norm over the 6 components) end the solve with DR_OK and
-                          dr_stop_reason() = DR_STOP_STAGNATION [1e-10; 0 = off].  It ends solves whose max-norm plateaus
-                          in near-void pores (contrast 1e-6) while C* is converged; DR_VOID_REL stays opt-in because
-                          it changes the moduli                                                                          */
+                          dr_stop_reason() = DR_STOP_STAGNATION [1e-10; 0 = off].  The movement is taken over at least 50
+                          iterations: checks closer than that to the last comparison are skipped by this rule, so the
+                          stop does not depend on DR_NCHECK when it is small (for DR_NCHECK >= 50 every check compares).
+                          It ends solves whose max-norm plateaus in near-void pores (contrast 1e-6) while C* is converged;
+                          DR_VOID_REL stays opt-in because it changes the moduli.  A solve ended this way returns DR_OK with
+                          a residual ABOVE tol: read dr_stop_reason / dr_info_lc to tell the two apart                     */
     DR_FORM = 8        /* 0 stress-relaxation form of the paper, Eq. 11-13 [default]; 1 displacement form: state u, w,
                           w <- (1-theta) w + C~^2 h^2 F(u)/H_node, u <- u + w, stresses formed on the fly (same fixed
                           point, 112 instead of 160 B per voxel-iteration; DR_KERNEL 0 or 1).  Setting DR_FORM also resets

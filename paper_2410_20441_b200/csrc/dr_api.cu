@@ -688,12 +688,21 @@ static dr_status averages(dr_handle* H, int lc, double eps0) {
 }
 
 // second stopping rule (Reading R9b): state of the <sigma> stagnation test of one solve
+// The movement is taken over at least DR_STAG_WINDOW iterations, whatever DR_NCHECK is: a check closer than that to the
+// last comparison is not `due` (with ncheck = 1 the per-iteration movement falls below stag_tol long before <sigma> has
+// converged).  For ncheck >= 50 every check compares.
+#define DR_STAG_WINDOW 50
 struct DrStag {
     bool have_prev = false;
     double prev[6] = {0, 0, 0, 0, 0, 0};
     int calm = 0;
-    // a[6] = <sigma> at this check; true when two consecutive checks moved <sigma> by <= stag_tol (relative, max-norm)
-    bool update(const double* a, double stag_tol) {
+    int prev_it = 0;
+    // does the check at iteration `it` take part in the rule (are its averages needed)?
+    bool due(int it) const { return !have_prev || it - prev_it >= DR_STAG_WINDOW; }
+    // a[6] = <sigma> at the check of iteration it (which is due); true when two consecutive comparisons moved <sigma> by
+    // <= stag_tol (relative, max-norm)
+    bool update(const double* a, double stag_tol, int it) {
+        prev_it = it;
         double num = 0.0, den = 0.0;
         for (int m = 0; m < 6; ++m) { num = std::max(num, std::fabs(a[m] - prev[m])); den = std::max(den, std::fabs(a[m])); }
         if (have_prev && num <= stag_tol * den) ++calm; else calm = 0;
@@ -732,14 +741,15 @@ extern "C" dr_status dr_solve(dr_handle* H, int lc, double eps0, double tol, int
         if (s != DR_OK) return s;
         if (chk) {
             // the averages of the stagnation rule ride on the same synchronisation as the residual
-            if (use_stag) { s = enqueue_averages(H, 9); if (s != DR_OK) return s; }
+            const bool sdue = use_stag && stag.due(it);
+            if (sdue) { s = enqueue_averages(H, 9); if (s != DR_OK) return s; }
             double r;
             s = read_residual(H, &r);
             if (s != DR_OK) return s;
             H->residual = r;
             if (!std::isfinite(r)) { status = DR_ERR_DIVERGED; H->stop_reason = DR_STOP_NONE; break; }
             if (r <= tol) { status = DR_OK; H->stop_reason = DR_STOP_RESIDUAL; break; }
-            if (use_stag && stag.update(H->pinned + 9, H->stag_tol)) { status = DR_OK; H->stop_reason = DR_STOP_STAGNATION; break; }
+            if (sdue && stag.update(H->pinned + 9, H->stag_tol, it)) { status = DR_OK; H->stop_reason = DR_STOP_STAGNATION; break; }
         }
     }
     H->iters = std::min(it, maxiter);
@@ -767,7 +777,7 @@ extern "C" dr_status dr_solve_six(dr_handle* const h[6], double eps0, double tol
     }
     DrPT P[6];
     int it[6];
-    bool active[6], pending[6];
+    bool active[6], pending[6], sdue[6] = {false, false, false, false, false, false};
     dr_status st[6];
     DrStag stag[6];
     for (int lc = 0; lc < 6; ++lc) {
@@ -796,7 +806,8 @@ extern "C" dr_status dr_solve_six(dr_handle* const h[6], double eps0, double tol
                 if (s != DR_OK) return s;
             }
             if (chk) {
-                if (H->stag_tol > 0.0) { dr_status s = enqueue_averages(H, 9); if (s != DR_OK) return s; }
+                sdue[lc] = H->stag_tol > 0.0 && stag[lc].due(it[lc]);
+                if (sdue[lc]) { dr_status s = enqueue_averages(H, 9); if (s != DR_OK) return s; }
                 CK(cudaMemcpyAsync(H->pinned + 8, H->res_bits, 8, cudaMemcpyDeviceToHost, H->st));
             }
             pending[lc] = chk;
@@ -813,7 +824,7 @@ extern "C" dr_status dr_solve_six(dr_handle* const h[6], double eps0, double tol
                 H->residual = r;
                 if (!std::isfinite(r)) { st[lc] = DR_ERR_DIVERGED; active[lc] = false; H->stop_reason = DR_STOP_NONE; H->err = "residual is not finite"; }
                 else if (r <= tol) { st[lc] = DR_OK; active[lc] = false; H->stop_reason = DR_STOP_RESIDUAL; }
-                else if (H->stag_tol > 0.0 && stag[lc].update(H->pinned + 9, H->stag_tol)) { st[lc] = DR_OK; active[lc] = false; H->stop_reason = DR_STOP_STAGNATION; }
+                else if (sdue[lc] && stag[lc].update(H->pinned + 9, H->stag_tol, it[lc])) { st[lc] = DR_OK; active[lc] = false; H->stop_reason = DR_STOP_STAGNATION; }
             }
             if (active[lc] && it[lc] >= maxiter) { active[lc] = false; H->err = "maxiter reached"; }
             any = any || active[lc];
@@ -904,7 +915,8 @@ extern "C" dr_status dr_solve_all(dr_handle* H, double eps0, double tol, int max
         { dr_status s = launch_coded(H, TB, ns, chk, n); if (s != DR_OK) return s; }
         for (int a = 0; a < ns; ++a) cur[slots[a]] ^= 1;
         if (!chk) continue;
-        if (use_stag) {
+        const bool sdue = use_stag && stag[slots[0]].due(it);     // the active load cases share their comparison history
+        if (sdue) {
             DrAvgSix A;
             for (int a = 0; a < ns; ++a) for (int f = 0; f < F_COUNT; ++f) A.F[a].f[f] = H->xbuf[slots[a]][cur[slots[a]]][f];
             k_avg_partial6<<<dim3(DR_AVG_BLOCKS, ns), DR_AVG_THREADS, 0, H->st>>>(H->L, A, H->partial6);
@@ -923,7 +935,7 @@ extern "C" dr_status dr_solve_all(dr_handle* H, double eps0, double tol, int max
             bool done = false;
             if (!std::isfinite(r)) { st[lc] = DR_ERR_DIVERGED; H->lc_stop[lc] = DR_STOP_NONE; done = true; }
             else if (r <= tol) { st[lc] = DR_OK; H->lc_stop[lc] = DR_STOP_RESIDUAL; done = true; }
-            else if (use_stag && stag[lc].update(H->pinned + 24 + 6 * a, H->stag_tol)) { st[lc] = DR_OK; H->lc_stop[lc] = DR_STOP_STAGNATION; done = true; }
+            else if (sdue && stag[lc].update(H->pinned + 24 + 6 * a, H->stag_tol, it)) { st[lc] = DR_OK; H->lc_stop[lc] = DR_STOP_STAGNATION; done = true; }
             if (done) { active[lc] = false; H->lc_iters[lc] = it; --nact; }
         }
     }

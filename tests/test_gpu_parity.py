@@ -298,8 +298,7 @@ def test_fields_191_default_chunking(oracle_mod, gpu, form):
     errs, ro, rs, ao, as_ = run_pair(oracle_mod, gpu, K, G, 4, 1e-4, 15, form=form)
     assert max(errs) <= FIELD_TOL, errs
     assert abs(ro - rs) <= 1e-9 * ro
-    # averages at this size: tests/test_gpu_configs.py measures which side carries the rounding (the oracle's sequential sum)
-    assert np.max(np.abs(ao - as_)) <= 1e-9 * np.max(np.abs(ao))
+    assert np.max(np.abs(ao - as_)) <= 1e-10 * np.max(np.abs(ao))
 
 
 def _fuzz_case(rng):
@@ -382,14 +381,14 @@ def test_palette_path_is_bitwise_the_fp64_path(gpu):
 # ---------------------------------------------------------------- round-2 additions: stopping rule, parameter hygiene
 def test_stagnation_rule_same_stop_as_oracle(oracle_mod, gpu):
     """Reading R9b: 48^3 pores at 1e-6 contrast plateau near 1e-5; both sides stop on <sigma> stagnation with DR_OK, the
-    same C, and (the decision compares 1e-10 changes, the sums differ at 1e-13) at most one check apart."""
+    same C, at the same check (both sides evaluate Eq. 7 to working precision, reading R7b)."""
     K, G, m = inputs.config3_random_spheres(n=48, npores=30, rmin=2.0, rmax=5.0, seed=7)
     s = gpu.Solver(to_dev(K), to_dev(G), ncheck=100)
     o = oracle_mod.Oracle(K, G, ncheck=100)
     for lc in (0, 3):
         assert s.solve(lc, 1e-4, 1e-8, 4800) == 0 and o.solve(lc, 1e-4, 1e-8, 4800) == 0
         assert s.stop_reason() == gpu.STOP_STAGNATION and o.stop_reason() == oracle_mod.STOP_STAGNATION
-        assert abs(s.info()[0] - o.info()[0]) <= 100 and s.info()[0] < 4800
+        assert s.info()[0] == o.info()[0] and s.info()[0] < 4800, (s.info(), o.info())
         assert np.max(np.abs(s.avg_stress() - o.avg_stress())) <= C_TOL * np.max(np.abs(o.avg_stress()))
     # rule off -> soft DR_MAXITER, same column
     s0 = gpu.Solver(to_dev(K), to_dev(G), ncheck=100, stag_tol=0.0)

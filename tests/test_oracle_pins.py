@@ -499,11 +499,46 @@ def test_stagnation_rule_stops_on_the_fixed_point_when_the_residual_plateaus(ora
     o2 = oracle_mod.Oracle(K, G, ncheck=20, stag_tol=0.0)
     assert o2.solve(2, 1e-4, 1e-8, 1500) == oracle_mod.MAXITER and o2.stop_reason() == oracle_mod.STOP_MAXITER
     assert np.max(np.abs(o2.avg_stress() / 1e-4 - Cb[:, 2])) <= 1e-8 * np.max(Cb)
+    # the stop does not hinge on ncheck: the movement is taken over >= 50 iterations, so frequent checks (ncheck 1, 2, 7) stop
+    # within one window of the ncheck = 50 solve (300 iterations) instead of as soon as the per-ITERATION movement is small
+    # (161 / 170 / 196 iterations before the window), and no further from the dense solve than it
+    ref = oracle_mod.Oracle(K, G, ncheck=50)
+    assert ref.solve(2, 1e-4, 1e-8, 6000) == 0 and ref.info()[0] == 300
+    e50 = np.max(np.abs(ref.avg_stress() / 1e-4 - Cb[:, 2]))
+    for nc in (1, 2, 7):
+        on = oracle_mod.Oracle(K, G, ncheck=nc)
+        assert on.solve(2, 1e-4, 1e-8, 6000) == 0 and on.stop_reason() == oracle_mod.STOP_STAGNATION
+        assert 300 <= on.info()[0] <= 350, (nc, on.info())
+        assert np.max(np.abs(on.avg_stress() / 1e-4 - Cb[:, 2])) <= 1.001 * e50
     # where the residual does reach tol the rule never fires first (same iteration counts as the survey probe: P14)
     Kh, Gh, _ = inputs.config1_sphere(n=16, r=3.0)
     a = oracle_mod.Oracle(Kh, Gh); b = oracle_mod.Oracle(Kh, Gh, stag_tol=0.0)
     assert a.solve(1, 1e-4, 1e-8, 5000) == 0 and b.solve(1, 1e-4, 1e-8, 5000) == 0
     assert a.info()[0] == b.info()[0] and a.stop_reason() == oracle_mod.STOP_RESIDUAL
+
+
+def test_volume_averages_equal_the_exact_sum_of_the_exported_fields(oracle_mod):
+    """Reading R7b: Eq. 7 is an exact sum and the oracle evaluates it to fp64 working precision (long double running sums).
+    After 40 iterations of the xz shear test on the 191 x 2 x 191 layered medium (one non-zero component) and on a ragged
+    voxel-noise image (all six non-zero) every <sigma_m> equals math.fsum of the weighted exported field -- the correctly
+    rounded sum -- to 1e-15 of the largest component; a dropped weight or a shifted edge index would not."""
+    import math
+    for (K, G, _), nonzero in ((inputs.layered(191, 2, 191), 1), (inputs.random_two_phase((60, 37, 41), seed=12), 6)):
+        o = oracle_mod.Oracle(K, G)
+        o.step(4, 1e-4, 40)
+        got = o.avg_stress()
+        N = K.size
+        exact = np.zeros(6)
+        for m, f in enumerate((3, 4, 5, 6, 7, 8)):
+            w = o.get_field(f).copy()
+            for d in {3: (0, 1), 4: (0, 2), 5: (1, 2)}.get(m, ()):      # tyz: weights 1/2 on first/last k, j; txz: k, i; txy: j, i
+                sl = [slice(None)] * 3
+                sl[d] = 0; w[tuple(sl)] *= 0.5
+                sl[d] = -1; w[tuple(sl)] *= 0.5
+            exact[m] = math.fsum(w.ravel().tolist()) / N
+        scale = np.max(np.abs(exact))
+        assert scale > 0 and np.count_nonzero(np.abs(exact) > 1e-9 * scale) >= nonzero, exact
+        assert np.max(np.abs(got - exact)) <= 1e-15 * scale, (got, exact)
 
 
 # ---------------------------------------------------------------- ABI behaviour
