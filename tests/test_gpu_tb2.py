@@ -193,7 +193,7 @@ def test_solve_all_fallback_reports_every_load_case_after_a_hard_error(gpu):
 
 
 def test_run_to_run_bitwise_determinism_and_kernel_equality_at_191(gpu):
-    """compute-sanitizer's racecheck is not available on the GPU pool, so races in the shared-memory pipeline of the two-iteration
+    """compute-sanitizer is closed on the GPU pool (profiles/r3_sanitizer.txt holds its output), so races in the shared-memory pipeline of the two-iteration
     kernel are hunted the other way: at 191^3 (560 CTAs of 512 threads, 4 waves, every tile shape) five runs of 60 iterations
     are identical bit for bit, and identical to the one-sweep kernel, whose staging, barriers and thread-to-node map differ."""
     import torch
