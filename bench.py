@@ -133,6 +133,35 @@ def make_image(workload, n_override=None, with_mask=False):
     return (K, G, n, m) if with_mask else (K, G, n)
 
 
+STOP_NAMES = ("none", "residual", "stagnation", "maxiter")
+# cfg 4 whole solve to tol 1e-8, default parameters: iterations per load case measured in round 2 with this kernel
+# (`bench.py --workload cfg4 --time-to-solution`: 133.4 s) -- used for a PROJECTION only
+CFG4_ITERS_R2 = (9500, 9500, 10000, 7200, 7800, 7500)
+
+
+def time_to_full_C_cfg2(torch, binding, dev, stream, eps0, tol, ncheck):
+    """BASELINE.json's third metric ("time to full 6x6 C_eff") inside the default, driver-run line: cfg 2 (191^3) from
+    dr_create to the 6x6 read-back with all six load cases in every launch (dr_solve_all), solved to `tol`; second of two
+    calls (the first warms up).  Every DR_OK carries the rule that produced it (dr_info_lc: residual or stagnation)."""
+    K2, G2, n2 = make_image("cfg2")
+    Kd2, Gd2 = torch.from_numpy(K2).to(dev), torch.from_numpy(G2).to(dev)
+    ws6 = torch.empty(binding.workspace_bytes(n2, n2, n2, True), dtype=torch.uint8, device=dev)
+    for rep in range(2):
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        b = binding.Solver(Kd2, Gd2, stream=stream, workspace=ws6, six=True, ncheck=ncheck)
+        C2, log2 = b.solve_all_batched(eps0, tol, 100 * n2)
+        torch.cuda.synchronize(dev)
+        dt = time.perf_counter() - t0
+        kern = b.active_kernel()
+        b.close()
+    return {"workload": "cfg2: " + WORKLOADS["cfg2"]["desc"], "seconds_incl_create": dt, "tol": tol, "ncheck": ncheck,
+            "driver": "dr_create + dr_solve_all (six load cases per launch) + dr_effective_C", "kernel": KERNEL_NAMES[kern],
+            "iters": [l[1] for l in log2], "status": [l[0] for l in log2], "residual": [l[2] for l in log2],
+            "stop": [STOP_NAMES[l[3]] for l in log2],
+            "C": [[float("%.6f" % v) for v in row] for row in C2]}
+
+
 def crop(K, G, m):
     m = min(m, K.shape[0])
     return np.ascontiguousarray(K[:m, :m, :m]), np.ascontiguousarray(G[:m, :m, :m]), m
@@ -225,6 +254,7 @@ def main():
     ap.add_argument("--direct-offdiag", action="store_true", help="time-to-solution: also run the 7th (triaxial) test and report Eq. 27-29")
     ap.add_argument("--st-factor", type=float, default=1.0, help="DR_ST_FACTOR (non-default tuning: 0.7 needs ~35 %% fewer iterations at 479^3)")
     ap.add_argument("--void-rel", type=float, default=0.0, help="DR_VOID_REL (non-default: exact-void clamp of near-void cells)")
+    ap.add_argument("--no-cfg2-tts", action="store_true", help="skip the cfg 2 time-to-full-6x6 block of the default line (~5 s)")
     ap.add_argument("--tts-maxiter-n", type=int, default=100, help="time-to-solution: maxiter = this x n per load case")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -285,13 +315,19 @@ def main():
         pal_active = s.uses_palette()
         ms = e0.elapsed_time(e1)
         # ---- dominant kernel alone (k_pt_fused back to back, no residual): average launch duration
-        s.iterate(lc, args.eps0, 5)
+        # an EVEN count, so that with two iterations per sweep every launch in the window is a pair (an odd count would mix a
+        # single-iteration launch in); the launch duration is the window divided by the launches the library counted
+        nk = args.steps + (args.steps & 1)
+        s.iterate(lc, args.eps0, 6)
+        lk0 = s.launch_count()
         k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         k0.record(stream)
-        s.iterate(lc, args.eps0, args.steps)
+        s.iterate(lc, args.eps0, nk)
         k1.record(stream)
         torch.cuda.synchronize(dev)
-        kms = k0.elapsed_time(k1) / args.steps
+        klaunches = max(int(s.launch_count() - lk0), 1)
+        kms = k0.elapsed_time(k1) / nk
+        launch_ms = k0.elapsed_time(k1) / klaunches
         clocks = sampler.stop() if rank == 0 else None
         active_kernel = s.active_kernel()
         # ---- sustained: what a real solve gets.  >= 3 s of back-to-back PT iterations (no residual check, no host sync) with
@@ -311,6 +347,7 @@ def main():
         if dist is not None:
             ms = shard.max_over_ranks(ms, dist, dev)
             kms = shard.max_over_ranks(kms, dist, dev)
+            launch_ms = shard.max_over_ranks(launch_ms, dist, dev)
 
         # ---- e2e through the C-ABI call with HOST buffers (H2D of K,G and D2H of C inside the timed region)
         # every rank runs the call on its own GPU (N independent images: weak scaling); time = max over ranks
@@ -400,20 +437,27 @@ def main():
                                   "iters": [l[1] for l in logb], "status": [l[0] for l in logb],
                                   "max_abs_dC_vs_sequential": float(np.max(np.abs(Cb - C)))}
 
+        cfg2_tts = None
+        if rank == 0 and world == 1 and args.workload == "cfg4" and args.n is None and not args.no_cfg2_tts and not args.time_to_solution:
+            cfg2_tts = time_to_full_C_cfg2(torch, binding, dev, stream, args.eps0, args.tol, args.ncheck)
+
     peak, peak_src = measured_peak()
     bpv = 112.0 if args.form == 1 else BYTES_PER_VOXEL_ITER      # algorithmic bytes per voxel-iteration of the form
     value = shard.job_throughput(N, args.steps, world, ms)
     teff = bpv * N * args.steps / (ms * 1e-3) / 1e9
     # one launch of the dominant kernel advances N voxels by `ipl` iterations: algorithmic bytes per launch = ipl x bpv x N
-    ipl = 2 if active_kernel == 3 else 1
-    launch_ms = kms * ipl
+    # (counted, not assumed: iterations of the window / launches of the window)
+    ipl = nk // klaunches
+    assert ipl * klaunches == nk and ipl == (2 if active_kernel == 3 else 1), (nk, klaunches, active_kernel)
     kern_gbs = ipl * bpv * N / (launch_ms * 1e-3) / 1e9
     traffic = ncu_traffic(args.workload, active_kernel, int(pal_active), args.form) if args.n is None else None
     roof = {"bound": "hbm", "kernel": KERNEL_NAMES[active_kernel], "achieved": kern_gbs, "peak": peak, "unit": "GB/s", "frac": kern_gbs / peak,
+            "algorithmic_frac": kern_gbs / peak, "launches_timed": klaunches, "iterations_timed": nk,
             "traffic": traffic, "peak_source": peak_src, "launch_ms": launch_ms, "iterations_per_launch": ipl,
             "algorithmic_bytes_per_launch": ipl * bpv * N,
             "note": "achieved = ALGORITHMIC bytes (160 B per voxel-iteration, SURVEY 8(d)) / launch time: with two iterations per sweep it "
-                    "may exceed the DRAM rate; physical = ncu dram bytes / launch time"}
+                    "may exceed the DRAM rate (frac = algorithmic_frac > 1 is not a DRAM rate); physical_frac = ncu dram bytes / launch time / peak "
+                    "is the figure bounded by 1"}
     if traffic is not None:
         roof["physical_GBs"] = traffic / (launch_ms * 1e-3) / 1e9
         roof["physical_frac"] = roof["physical_GBs"] / peak
@@ -442,6 +486,14 @@ def main():
         line["sustained"] = sustained
     if tts is not None:
         line["time_to_full_C"] = tts
+    elif cfg2_tts is not None:
+        line["time_to_full_C"] = cfg2_tts
+        if sustained is not None and args.form == 0 and args.kernel == 3:
+            line["cfg4_projection"] = {
+                "label": "projected, not measured in this run",
+                "seconds": sum(CFG4_ITERS_R2) * sustained["ms_per_step"] * 1e-3,
+                "how": "sum of the iterations per load case of the round-2 whole solve of cfg 4 to tol 1e-8 (BASELINE.md section 5: "
+                       "%s, measured 133.4 s) x this line's sustained ms_per_step" % (list(CFG4_ITERS_R2),)}
     if not args.no_cpu_baseline:
         rate, dt, m = oracle_rate(K, G, lc, args.eps0, args.cpu_sample_n, args.cpu_iters)
         line["cpu_baseline"] = {"value": rate, "unit": "voxel-updates/s", "cores": host_threads(), "kind": "oracle",

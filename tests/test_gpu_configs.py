@@ -79,6 +79,20 @@ def test_cfg2_converged_C_vs_oracle_and_contribution_tensor(oracle_mod, gpu):
     assert abs(C[0, 0] - C[1, 1]) <= 1e-9 * s0 and abs(C[0, 2] - C[1, 2]) <= 1e-9 * s0 and abs(C[3, 3] - C[4, 4]) <= 1e-9 * s0
     assert C[2, 2] < C[0, 0] and C[3, 3] < C[5, 5]          # softest across the thin (z) direction of the oblate inclusion
     s.close()
+    # the launch geometry behind BASELINE.md's 2.1 s for this config: six load cases per launch at 191^3 (560 tiles x 6 slots x
+    # z chunks in blockIdx.z) and six handles on six streams -- the same bits as the sequential solves above, hence the
+    # same distance to the oracle columns
+    b = gpu.Solver(to_dev(K), to_dev(G), six=True, ncheck=100)
+    Cb, logb = b.solve_all_batched(1e-4, 1e-8, 19100)
+    assert b.active_kernel() == 3
+    assert [(l[0], l[1], l[3]) for l in logb] == [(l[0], l[1], l[4]) for l in log], (logb, log)
+    assert np.array_equal(Cb, C)
+    b.close(); del b
+    C6, log6, solvers = gpu.solve_six(to_dev(K), to_dev(G), eps0=1e-4, tol=1e-8, maxiter=19100, ncheck=100)
+    assert [(l[0], l[1]) for l in log6] == [(l[0], l[1]) for l in log] and np.array_equal(C6, C)
+    for sv in solvers:
+        sv.close()
+    del solvers
     # matrix-only run = Hooke (pin P1), solved on the GPU as the config asks
     K1, G1 = inputs.homogeneous(191, 70.2, 29.0)
     s1 = gpu.Solver(to_dev(K1), to_dev(G1), ncheck=100)
